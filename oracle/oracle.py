@@ -1,0 +1,126 @@
+"""ctypes front end of the float64 CPU oracle (oracle/synim_oracle.c).
+
+TEST INFRASTRUCTURE, NOT PRODUCT CODE: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this module.  It shares
+nothing with the CUDA path (paper_2606_07759_b200/csrc) and never imports it.
+See the header of synim_oracle.c for the passages of PAPER.md each step follows.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "synim_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+ND, GTILT = 0, 1
+
+#: order of the physical parameters in the double[15] record synim_oracle_compose reads
+_FIELDS = ("shift_x", "shift_y", "rot_deg", "mag_x", "mag_y",
+           "dm_shift_x", "dm_shift_y", "dm_rot_deg", "dm_mag",
+           "dm_height_m", "gs_range_m", "gs_theta_arcsec", "gs_azimuth_deg",
+           "src_pixel_pitch_m", "wfs_pitch_src_px")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain C, OpenMP over modes)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
+                               "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        f64p = ctypes.POINTER(ctypes.c_double)
+        lib.synim_oracle_wfs.restype = ctypes.c_int
+        lib.synim_oracle_wfs.argtypes = [
+            ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+            ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, f64p, ctypes.c_double,
+            ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p]
+        lib.synim_oracle_resample.restype = ctypes.c_int
+        lib.synim_oracle_resample.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                              f64p, ctypes.c_int32, ctypes.c_void_p]
+        lib.synim_oracle_compose.restype = ctypes.c_int
+        lib.synim_oracle_compose.argtypes = [f64p, f64p]
+        lib.synim_oracle_num_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().synim_oracle_num_threads())
+
+
+def compose_affine(phys: dict) -> np.ndarray:
+    """Physical parameters -> composite 2x3 matrix a[6] (output -> input, centred pixels)."""
+    p = (ctypes.c_double * 15)(*[float(phys[k]) for k in _FIELDS])
+    a = (ctypes.c_double * 6)()
+    if _load().synim_oracle_compose(p, a) != 0:
+        raise ValueError("oracle: bad physical parameters")
+    return np.array(list(a), dtype=np.float64)
+
+
+def resample(g: np.ndarray, m: int, a: Sequence[float], halo: bool = False) -> np.ndarray:
+    """The resampled screen of one mode (steps 1-2), float64: [M][M], or with ``halo`` the
+    [M+2][M+2] grid of pixels -1..M."""
+    g = np.ascontiguousarray(g, dtype=np.float32)
+    out = np.empty((m + 2, m + 2) if halo else (m, m), dtype=np.float64)
+    aa = (ctypes.c_double * 6)(*[float(v) for v in a])
+    rc = _load().synim_oracle_resample(g.ctypes.data, g.shape[0], g.shape[1], m, aa, int(halo),
+                                       out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle resample failed ({rc})")
+    return out
+
+
+def slopes_wfs(cube: np.ndarray, pupil: np.ndarray, n_subap: int, n_pix: int, valid: np.ndarray,
+               a: Sequence[float], scale: float = 1.0, mode: int = ND,
+               modes: Optional[Sequence[int]] = None, n_threads: int = 0) -> np.ndarray:
+    """Slopes of the selected modes for one WFS: float64 [n_sel][2*n_valid] (x then y)."""
+    cube = np.ascontiguousarray(cube, dtype=np.float32)
+    pupil = np.ascontiguousarray(pupil, dtype=np.float32)
+    valid = np.ascontiguousarray(valid, dtype=np.uint8)
+    n_tot, ny, nx = cube.shape
+    assert pupil.shape == (n_subap * n_pix, n_subap * n_pix) and valid.shape == (n_subap, n_subap)
+    if modes is None:
+        idx_p, n_sel = None, n_tot
+    else:
+        idx = np.ascontiguousarray(modes, dtype=np.int32)
+        idx_p, n_sel = idx.ctypes.data, idx.size
+    nv = int(valid.sum())
+    out = np.zeros((n_sel, 2 * nv), dtype=np.float64)
+    aa = (ctypes.c_double * 6)(*[float(v) for v in a])
+    rc = _load().synim_oracle_wfs(cube.ctypes.data, n_tot, idx_p, n_sel, ny, nx, pupil.ctypes.data,
+                                  n_subap, n_pix, valid.ctypes.data, aa, float(scale), int(mode),
+                                  int(n_threads), out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle failed ({rc})")
+    return out
+
+
+def interaction_matrix(wl, mode: int = ND, modes: Optional[Sequence[int]] = None,
+                       wfs: Optional[Sequence[int]] = None, n_threads: int = 0,
+                       affines: Optional[Sequence[Sequence[float]]] = None) -> np.ndarray:
+    """IM of a workload: float64 [rows][n_sel], rows = WFS 0..n-1, each x slopes then y slopes.
+
+    ``wfs`` restricts to some sensors (rows of the others are left out);
+    ``affines`` overrides the composite matrices (else composed from ``phys``)."""
+    sel = list(range(len(wl.wfs))) if wfs is None else list(wfs)
+    blocks = []
+    for k in sel:
+        w = wl.wfs[k]
+        a = compose_affine(w.phys) if affines is None else affines[k]
+        blocks.append(slopes_wfs(wl.cube, w.pupil, w.n_subap, w.n_pix, w.valid, a, w.slope_scale,
+                                 mode, modes, n_threads).T)
+    return np.concatenate(blocks, axis=0)

@@ -1,0 +1,343 @@
+"""Seeded synthetic inputs for the five BASELINE.json configurations.
+
+This module is the ONLY code shared by the CUDA path and the oracle.  It holds
+none of the method's arithmetic: no affine composition, no interpolation, no
+slopes.  It only manufactures the *inputs* of the synthetic interaction-matrix
+computation (section 2.1-2.2):
+
+  * the influence-function cube ``[n_modes][ny][nx]`` float32 (zonal Gaussian
+    actuators or Zernike modes) and, for zonal cubes, the tight non-zero
+    bounding box of every influence function,
+  * per wavefront sensor: the Shack-Hartmann subaperture grid, the pupil
+    weights in the WFS frame, the valid-subaperture mask, and the *physical*
+    misregistration / guide-star parameters.  Turning those parameters into a
+    composite affine matrix is method arithmetic and is done
+    separately by each side (``synim_compose_affine`` in the library,
+    ``oracle_compose_affine`` in the oracle).
+
+The real MORFEO influence functions, modal bases and YAML files the paper
+measures on are not available; these inputs stand in
+for them with the same shapes, sizes and structure ("Input
+recipe").  Everything is generated in float64 and cast to float32 once.
+Seeds are ``7759 + cfg``.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+ARCSEC = math.pi / (180.0 * 3600.0)
+
+#: keys of the physical parameter record of one WFS (all float64); the same
+#: field list as ``synim_wfs_physical`` in include/synim.h.
+PHYSICAL_FIELDS = (
+    "shift_x", "shift_y", "rot_deg", "mag_x", "mag_y",
+    "dm_shift_x", "dm_shift_y", "dm_rot_deg", "dm_mag",
+    "dm_height_m", "gs_range_m", "gs_theta_arcsec", "gs_azimuth_deg",
+    "src_pixel_pitch_m", "wfs_pitch_src_px",
+)
+
+
+def physical(**kw) -> dict:
+    """A physical-parameter record with neutral defaults."""
+    p = dict(shift_x=0.0, shift_y=0.0, rot_deg=0.0, mag_x=1.0, mag_y=1.0,
+             dm_shift_x=0.0, dm_shift_y=0.0, dm_rot_deg=0.0, dm_mag=1.0,
+             dm_height_m=0.0, gs_range_m=math.inf, gs_theta_arcsec=0.0,
+             gs_azimuth_deg=0.0, src_pixel_pitch_m=1.0, wfs_pitch_src_px=1.0)
+    for k, v in kw.items():
+        if k not in p:
+            raise KeyError(k)
+        p[k] = float(v)
+    return p
+
+
+@dataclass
+class WfsInput:
+    n_subap: int
+    n_pix: int
+    pupil: np.ndarray        # float32 [M][M], M = n_subap*n_pix, weights in the WFS frame
+    valid: np.ndarray        # uint8 [n_subap][n_subap], 1 = valid
+    phys: dict               # PHYSICAL_FIELDS -> float
+    slope_scale: float = 1.0
+
+    @property
+    def m(self) -> int:
+        return self.n_subap * self.n_pix
+
+    @property
+    def n_valid(self) -> int:
+        return int(self.valid.sum())
+
+
+@dataclass
+class Workload:
+    name: str
+    cfg: int
+    ny: int
+    nx: int
+    cube: np.ndarray                 # float32 [n_modes][ny][nx]
+    bbox: Optional[np.ndarray]       # int32 [n_modes][4] (x0,y0,x1,y1 inclusive) or None (dense)
+    wfs: List[WfsInput] = field(default_factory=list)
+    mode_ids: Optional[np.ndarray] = None   # index of each kept mode in the full config
+
+    @property
+    def n_modes(self) -> int:
+        return int(self.cube.shape[0])
+
+    @property
+    def n_rows(self) -> int:
+        return 2 * sum(w.n_valid for w in self.wfs)
+
+    @property
+    def n_columns(self) -> int:
+        """IM columns in the metric's sense: one per (mode, WFS) pair."""
+        return self.n_modes * len(self.wfs)
+
+
+# --------------------------------------------------------------------------
+# pupil, subapertures
+# --------------------------------------------------------------------------
+def make_pupil(m: int, diameter: float, obstruction: float) -> np.ndarray:
+    """Binary annular pupil on an m x m grid, pixel k at k-(m-1)/2."""
+    c = (m - 1) / 2.0
+    y, x = np.mgrid[0:m, 0:m].astype(np.float64)
+    r = np.hypot(x - c, y - c)
+    p = (r <= diameter / 2.0) & (r >= obstruction * diameter / 2.0)
+    return p.astype(np.float32)
+
+
+def valid_subaps(pupil: np.ndarray, n_subap: int, n_pix: int, min_frac: float = 0.5) -> np.ndarray:
+    """Subaperture (a,b) is valid iff its summed weight >= min_frac*n_pix^2 (ties valid)."""
+    s = pupil.astype(np.float64).reshape(n_subap, n_pix, n_subap, n_pix).sum(axis=(1, 3))
+    return (s >= min_frac * n_pix * n_pix).astype(np.uint8)
+
+
+# --------------------------------------------------------------------------
+# zonal Gaussian influence functions
+# --------------------------------------------------------------------------
+def actuator_grid(n_act: int, pitch: float, r_keep: float) -> np.ndarray:
+    """Centred positions (x,y) of the n_act x n_act actuators kept (r <= r_keep), row-major."""
+    u = (np.arange(n_act) - (n_act - 1) / 2.0) * pitch
+    yy, xx = np.meshgrid(u, u, indexing="ij")
+    keep = np.hypot(xx, yy) <= r_keep
+    return np.stack([xx[keep], yy[keep]], axis=1)
+
+
+def gaussian_cube(ny: int, nx: int, act_xy: np.ndarray, pitch: float,
+                  coupling: float = 0.3, support_pitches: float = 3.0):
+    """Gaussian influence functions exp(ln(coupling) r^2/pitch^2), zero for r > support*pitch.
+
+    Returns (cube float32 [n][ny][nx], bbox int32 [n][4] tight non-zero extent)."""
+    n = act_xy.shape[0]
+    cube = np.zeros((n, ny, nx), dtype=np.float32)
+    bbox = np.zeros((n, 4), dtype=np.int32)
+    cx, cy = (nx - 1) / 2.0, (ny - 1) / 2.0
+    rad = support_pitches * pitch
+    lnc = math.log(coupling)
+    for k in range(n):
+        ax, ay = act_xy[k, 0] + cx, act_xy[k, 1] + cy     # actuator centre in pixel indices
+        x0 = max(0, int(math.floor(ax - rad)))
+        x1 = min(nx - 1, int(math.ceil(ax + rad)))
+        y0 = max(0, int(math.floor(ay - rad)))
+        y1 = min(ny - 1, int(math.ceil(ay + rad)))
+        if x1 < x0 or y1 < y0:
+            bbox[k] = (0, 0, -1, -1)
+            continue
+        ys, xs = np.mgrid[y0:y1 + 1, x0:x1 + 1].astype(np.float64)
+        r2 = (xs - ax) ** 2 + (ys - ay) ** 2
+        patch = np.where(r2 <= rad * rad, np.exp(lnc * r2 / (pitch * pitch)), 0.0).astype(np.float32)
+        cube[k, y0:y1 + 1, x0:x1 + 1] = patch
+        nz_r = np.flatnonzero(patch.any(axis=1))
+        nz_c = np.flatnonzero(patch.any(axis=0))
+        if nz_r.size == 0:
+            bbox[k] = (0, 0, -1, -1)
+        else:
+            bbox[k] = (x0 + nz_c[0], y0 + nz_r[0], x0 + nz_c[-1], y0 + nz_r[-1])
+    return cube, bbox
+
+
+def tight_bboxes(cube: np.ndarray) -> np.ndarray:
+    """Tight non-zero extent of every mode: (x0,y0,x1,y1) inclusive; (0,0,-1,-1) if all zero."""
+    n = cube.shape[0]
+    out = np.zeros((n, 4), dtype=np.int32)
+    for k in range(n):
+        nz = cube[k] != 0
+        r = np.flatnonzero(nz.any(axis=1))
+        c = np.flatnonzero(nz.any(axis=0))
+        out[k] = (c[0], r[0], c[-1], r[-1]) if r.size else (0, 0, -1, -1)
+    return out
+
+
+# --------------------------------------------------------------------------
+# Zernike modes (Noll ordering), stable to high radial order
+# --------------------------------------------------------------------------
+def noll_to_nm(j: int):
+    """Noll index j>=1 -> (n, m) with m>0 for the cosine and m<0 for the sine term."""
+    n = 0
+    while (n + 1) * (n + 2) // 2 < j:
+        n += 1
+    p = j - n * (n + 1) // 2 - 1                 # 0..n inside radial order n
+    am = 2 * ((p + 1) // 2) if n % 2 == 0 else 2 * (p // 2) + 1
+    if am == 0:
+        return n, 0
+    return (n, am) if j % 2 == 0 else (n, -am)
+
+
+def _radial_family(rho: np.ndarray, m: int, n_max: int):
+    """Yield (n, R_n^m(rho)) for n = m, m+2, ... <= n_max.
+
+    R_n^m(rho) = rho^m P_k^{(0,m)}(2 rho^2 - 1), k = (n-m)/2, with the Jacobi
+    three-term recurrence (the factorial sum loses all digits beyond n ~ 40)."""
+    x = 2.0 * rho * rho - 1.0
+    rm = rho ** m
+    a, b = 0.0, float(m)
+    p_prev = np.ones_like(x)
+    yield m, rm * p_prev
+    if m + 2 > n_max:
+        return
+    p_cur = 0.5 * ((a - b) + (a + b + 2.0) * x)
+    yield m + 2, rm * p_cur
+    k = 2
+    while m + 2 * k <= n_max:
+        c = 2.0 * k + a + b
+        a1 = 2.0 * k * (k + a + b) * (c - 2.0)
+        a2 = (c - 1.0) * (a * a - b * b)
+        a3 = (c - 2.0) * (c - 1.0) * c
+        a4 = 2.0 * (k + a - 1.0) * (k + b - 1.0) * c
+        p_next = ((a2 + a3 * x) * p_cur - a4 * p_prev) / a1
+        p_prev, p_cur = p_cur, p_next
+        yield m + 2 * k, rm * p_cur
+        k += 1
+
+
+def zernike_cube(ny: int, nx: int, radius: float, pupil_src: np.ndarray,
+                 j_first: int, j_last: int, j_keep: Optional[Sequence[int]] = None) -> np.ndarray:
+    """Zernike modes Noll j_first..j_last on the source grid, unit RMS over ``pupil_src`` pixels.
+
+    rho is clamped to 1 outside the unit disc (the polynomials explode beyond it)."""
+    js = list(range(j_first, j_last + 1)) if j_keep is None else list(j_keep)
+    slot = {j: i for i, j in enumerate(js)}
+    cube = np.zeros((len(js), ny, nx), dtype=np.float32)
+    cx, cy = (nx - 1) / 2.0, (ny - 1) / 2.0
+    yy, xx = np.mgrid[0:ny, 0:nx].astype(np.float64)
+    rho = np.minimum(np.hypot(xx - cx, yy - cy) / radius, 1.0)
+    theta = np.arctan2(yy - cy, xx - cx)
+    pmask = pupil_src > 0
+    want = {}
+    for j in js:
+        n, m = noll_to_nm(j)
+        want.setdefault(abs(m), {}).setdefault(n, []).append((j, m))
+    n_max = max(noll_to_nm(j)[0] for j in js)
+    for am, by_n in sorted(want.items()):
+        cosm = np.cos(am * theta) if am else None
+        sinm = np.sin(am * theta) if am else None
+        for n, rad in _radial_family(rho, am, n_max):
+            for (j, m) in by_n.get(n, ()):
+                z = rad if m == 0 else (rad * cosm if m > 0 else rad * sinm)
+                rms = math.sqrt(float(np.mean(z[pmask] ** 2)))
+                cube[slot[j]] = (z / rms).astype(np.float32)
+    return cube
+
+
+# --------------------------------------------------------------------------
+# the five configurations (BASELINE.json "configs")
+# --------------------------------------------------------------------------
+def _subset(n_total: int, max_modes: Optional[int], seed: int) -> np.ndarray:
+    if max_modes is None or max_modes >= n_total:
+        return np.arange(n_total)
+    rng = np.random.default_rng(seed + 1000)
+    return np.sort(rng.choice(n_total, size=max_modes, replace=False))
+
+
+def _cfg3_physical(seed: int):
+    """Per-WFS parameters of config 3 (also used by config 5): rot k*60+U(+-0.5) deg,
+    shift U(+-0.5) px, magnification 1+U(+-0.01); draw order rot, shift_x, shift_y, mag."""
+    rng = np.random.default_rng(seed)
+    out = []
+    for k in range(6):
+        rot = 60.0 * k + rng.uniform(-0.5, 0.5)
+        sx = rng.uniform(-0.5, 0.5)
+        sy = rng.uniform(-0.5, 0.5)
+        mag = 1.0 + rng.uniform(-0.01, 0.01)
+        out.append(physical(shift_x=sx, shift_y=sy, rot_deg=rot, mag_x=mag, mag_y=mag))
+    return out
+
+
+def make_config(cfg: int, max_modes: Optional[int] = None) -> Workload:
+    """Build configuration ``cfg`` (1..5).  ``max_modes`` keeps a seeded, sorted subset of
+    the modes (same WFS set) so that tests can run a structurally identical smaller case."""
+    seed = 7759 + cfg
+    if cfg == 1:
+        n, npix, nsub = 80, 8, 10
+        pup = make_pupil(n, 80.0, 0.14)
+        acts = actuator_grid(11, 8.0, 40.0 + 4.0)
+        keep = _subset(len(acts), max_modes, seed)
+        cube, bbox = gaussian_cube(n, n, acts[keep], 8.0)
+        w = WfsInput(nsub, npix, pup, valid_subaps(pup, nsub, npix),
+                     physical(shift_x=0.3, shift_y=-0.2, rot_deg=1.5, mag_x=1.02, mag_y=1.02))
+        return Workload("SCAO tiny", 1, n, n, cube, bbox, [w], keep)
+    if cfg == 2:
+        n, npix, nsub = 400, 10, 40
+        pup = make_pupil(n, 400.0, 0.14)
+        acts = actuator_grid(41, 10.0, 200.0 + 5.0)
+        keep = _subset(len(acts), max_modes, seed)
+        cube, bbox = gaussian_cube(n, n, acts[keep], 10.0)
+        rng = np.random.default_rng(seed)
+        sx, sy = rng.uniform(-0.5, 0.5), rng.uniform(-0.5, 0.5)
+        rot = rng.uniform(-2.0, 2.0)
+        mag = 1.0 + rng.uniform(-0.02, 0.02)
+        w = WfsInput(nsub, npix, pup, valid_subaps(pup, nsub, npix),
+                     physical(shift_x=sx, shift_y=sy, rot_deg=rot, mag_x=mag, mag_y=mag))
+        return Workload("VLT-class SCAO", 2, n, n, cube, bbox, [w], keep)
+    if cfg in (3, 5):
+        n, npix, nsub = 480, 7, 68
+        m = nsub * npix                                  # 476
+        pup = make_pupil(m, 476.0, 0.28)
+        val = valid_subaps(pup, nsub, npix)
+        wfs = [WfsInput(nsub, npix, pup, val, p) for p in _cfg3_physical(7759 + 3)]
+        if cfg == 3:
+            acts = actuator_grid(81, 6.0, 238.0 + 3.0)
+            keep = _subset(len(acts), max_modes, seed)
+            cube, bbox = gaussian_cube(n, n, acts[keep], 6.0)
+            return Workload("ELT MCAO ground DM, 6 LGS", 3, n, n, cube, bbox, wfs, keep)
+        keep = _subset(2000, max_modes, seed)
+        cube = zernike_cube(n, n, 238.0, make_pupil(n, 476.0, 0.28), 2, 2001,
+                            j_keep=[2 + int(k) for k in keep])
+        return Workload("Modal ELT IM, 2000 Zernikes, 6 LGS", 5, n, n, cube, None, wfs, keep)
+    if cfg == 4:
+        n = 600
+        pitch_m = 38.5 / 476.0
+        pup = make_pupil(476, 476.0, 0.28)
+        acts = actuator_grid(60, 10.0, 300.0 + 5.0)
+        keep = _subset(len(acts), max_modes, seed)
+        cube, bbox = gaussian_cube(n, n, acts[keep], 10.0)
+        wfs = []
+        val_l = valid_subaps(pup, 68, 7)
+        for k in range(6):
+            wfs.append(WfsInput(68, 7, pup, val_l, physical(
+                dm_height_m=17000.0, gs_range_m=90000.0, gs_theta_arcsec=45.0,
+                gs_azimuth_deg=60.0 * k, src_pixel_pitch_m=pitch_m)))
+        val_n = valid_subaps(pup, 2, 238)
+        for az in (90.0, 210.0, 330.0):
+            wfs.append(WfsInput(2, 238, pup, val_n, physical(
+                dm_height_m=17000.0, gs_range_m=math.inf, gs_theta_arcsec=80.0,
+                gs_azimuth_deg=az, src_pixel_pitch_m=pitch_m)))
+        return Workload("ELT MCAO altitude DM, 6 LGS + 3 NGS", 4, n, n, cube, bbox, wfs, keep)
+    raise ValueError(f"unknown config {cfg}")
+
+
+def random_smooth_cube(n_modes: int, ny: int, nx: int, seed: int) -> np.ndarray:
+    """Dense test modes: a few random low-order 2-D cosines per mode (no compact support)."""
+    rng = np.random.default_rng(seed)
+    yy, xx = np.mgrid[0:ny, 0:nx].astype(np.float64)
+    cube = np.empty((n_modes, ny, nx), dtype=np.float32)
+    for k in range(n_modes):
+        z = np.zeros((ny, nx))
+        for _ in range(4):
+            fx, fy = rng.uniform(-3, 3, size=2) * 2 * math.pi / max(nx, ny)
+            z += rng.normal() * np.cos(fx * xx + fy * yy + rng.uniform(0, 2 * math.pi))
+        cube[k] = z.astype(np.float32)
+    return cube

@@ -1,0 +1,158 @@
+/*
+ * synim.h -- C ABI of the B200-native synthetic Shack-Hartmann interaction-matrix engine.
+ *
+ * What the library computes (SynIM, arxiv/paper_2606_07759; citations are lines of
+ * /root/reference/PAPER.md, "R<n>" are the readings listed in DESIGN.md):
+ *
+ *   for every (mode m, wavefront sensor w)            -- one IM column in the metric's sense
+ *     1. ONE composite affine transform per WFS maps every WFS pixel to the DM / meta-pupil grid
+ *        (sec. 2.1: DM and WFS matrices "multiplied into a single composite matrix";
+ *        :47 altitude-dependent perspective scaling),
+ *     2. the influence function is bilinearly interpolated exactly once,
+ *        zero outside the grid (R4),
+ *     3. finite central differences at every WFS pixel (sec. 2.2),
+ *     4. spatial average over each valid subaperture, weighted by the pupil weights (PAPER.md:61,
+ *        :116), times the caller's slope scale,
+ *   assembled into IM[rows][n_modes], rows = 2 * sum_w n_valid_w.
+ *
+ * Conventions
+ *   - Pixel k of an N-pixel axis sits at k-(N-1)/2 (R2).  x = column direction, y = row direction.
+ *   - The composite matrix maps WFS pixel coordinates (x_w, y_w) to source-grid coordinates:
+ *       x_s = a[0]*x_w + a[1]*y_w + a[2],   y_s = a[3]*x_w + a[4]*y_w + a[5]        (R1)
+ *   - Row order inside a column: WFS 0..n_wfs-1; inside a WFS all x slopes of the valid
+ *     subapertures in row-major (a,b) order, then all y slopes (R9).
+ *   - The IM is column-major: element (r, m) is d_out[m*ld + r]  (float32).
+ *   - "HOST" / "DEVICE" say where a pointer lives.  The caller owns every buffer it passes in;
+ *     HOST arrays are consumed during the call and may be freed on return.  DEVICE buffers must
+ *     stay valid until the work enqueued on `stream` has finished.  The library owns only the
+ *     geometry object and its small internal device buffers.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls
+ *     enqueue work and return without synchronising unless stated otherwise.
+ *   - Every entry point returns a synim_status; nothing throws or aborts across the ABI.  There is
+ *     NO CPU fallback: without a CUDA device of compute capability 10.x the compute entry points
+ *     return SYNIM_ERR_UNSUPPORTED_DEVICE / SYNIM_ERR_CUDA.  synim_last_error() gives the text
+ *     of the calling thread's last failure.
+ */
+#ifndef SYNIM_H_
+#define SYNIM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SYNIM_VERSION_MAJOR 0
+#define SYNIM_VERSION_MINOR 1
+
+typedef struct synim_geometry synim_geometry; /* opaque, library-owned */
+
+typedef enum {
+    SYNIM_OK = 0,
+    SYNIM_ERR_INVALID_ARG = -1,        /* NULL pointer, non-positive size, ld < rows, singular matrix ... */
+    SYNIM_ERR_ALIGNMENT = -2,          /* cube pointer not 16-byte aligned or nx % 4 != 0 (TMA) */
+    SYNIM_ERR_EMPTY_SUBAP = -3,        /* a subaperture flagged valid has zero summed pupil weight */
+    SYNIM_ERR_UNSUPPORTED_DEVICE = -4, /* current device is not compute capability 10.x */
+    SYNIM_ERR_OUT_OF_MEMORY = -5,
+    SYNIM_ERR_CUDA = -6,               /* any other CUDA runtime / driver failure */
+    SYNIM_ERR_UNSUPPORTED = -7         /* feature not built on this path (see synim_slope_mode) */
+} synim_status;
+
+/* Slope estimator.  ND = finite central differences averaged over the subaperture
+ * (the paper's engine).  GTILT = boundary-driven telescoping sum: the first/last valid pixel
+ * (P >= 0.5) of every pixel row / column of the subaperture (R13). */
+typedef enum { SYNIM_SLOPES_ND = 0, SYNIM_SLOPES_GTILT = 1 } synim_slope_mode;
+
+/* One Shack-Hartmann sensor's static description.  M = n_subap*n_pix WFS pixels per side;
+ * subaperture (a,b) owns pixels i in [a*n_pix,(a+1)*n_pix), j in [b*n_pix,(b+1)*n_pix). */
+typedef struct {
+    int32_t n_subap;
+    int32_t n_pix;
+    const uint8_t *valid_mask;   /* HOST  [n_subap][n_subap] row-major, non-zero = valid (R10) */
+    const float *d_pupil;        /* DEVICE [M][M] row-major non-negative weights P in the WFS frame (R7) */
+} synim_wfs_grid;
+
+/* Per-call geometry of one sensor: the composite output->input matrix in centred pixel
+ * coordinates (see Conventions) and the factor every slope of this sensor is multiplied by (R8). */
+typedef struct {
+    double a[6];
+    double slope_scale;
+} synim_wfs_affine;
+
+/* Physical parameters the composite matrix is built from (R1, R11, R12).
+ * Lengths in source-grid pixels unless stated; angles as named.  Chain, WFS pixel -> source grid:
+ *   u1 = wfs_pitch_src_px * x_w - (shift_x, shift_y)
+ *   u2 = diag(1/mag_x, 1/mag_y) * R(-rot_deg) * u1
+ *   u3 = kappa * u2 + f,   kappa = 1 - dm_height_m/gs_range_m (1 if gs_range_m is +inf),
+ *                          f = dm_height_m * theta * (cos az, sin az) / src_pixel_pitch_m
+ *   x_s = (1/dm_mag) * R(-dm_rot_deg) * (u3 - (dm_shift_x, dm_shift_y))
+ * with R(-t) = [[cos t, sin t], [-sin t, cos t]]. */
+typedef struct {
+    double shift_x, shift_y, rot_deg, mag_x, mag_y;
+    double dm_shift_x, dm_shift_y, dm_rot_deg, dm_mag;
+    double dm_height_m, gs_range_m, gs_theta_arcsec, gs_azimuth_deg, src_pixel_pitch_m;
+    double wfs_pitch_src_px;
+} synim_wfs_physical;
+
+/* Pure host helper (no CUDA): compose the single matrix of PAPER.md:49 from physical parameters.
+ * out->slope_scale is set to 1.  SYNIM_ERR_INVALID_ARG on NULL, zero magnification or pitch <= 0. */
+synim_status synim_compose_affine(const synim_wfs_physical *phys, synim_wfs_affine *out);
+
+/* Build the static geometry for n_wfs sensors looking at an ny x nx source grid (S0 of SURVEY.md
+ * sec. 8(a)): per sensor the valid-subaperture row map, the per-pixel reduction weights
+ * 0.5*P/W_S (W_S = summed weight of the pixel's subaperture, 0 for invalid ones) and the row offsets
+ * of the sensor inside a column.  Runs small kernels on `stream` and SYNCHRONISES it once to
+ * report SYNIM_ERR_EMPTY_SUBAP.  grids[w].d_pupil is only read during this call.
+ * Requirements: 1 <= n_wfs <= 64, n_subap >= 1, n_pix >= 1, nx % 4 == 0. */
+synim_status synim_create_geometry(int32_t ny, int32_t nx, int32_t n_wfs, const synim_wfs_grid *grids,
+                                   void *stream, synim_geometry **out);
+
+/* rows of the IM = 2 * sum_w n_valid_w; -1 on NULL. */
+int64_t synim_num_rows(const synim_geometry *geom);
+/* number of valid subapertures of sensor w, and the row where its x slopes start; -1 on error. */
+int64_t synim_num_valid(const synim_geometry *geom, int32_t wfs);
+int64_t synim_row_offset(const synim_geometry *geom, int32_t wfs);
+
+/* The hot path (S1-S4): all (mode, WFS) pairs, fused coordinate generation, shared-memory gather of
+ * TMA-staged influence-function tiles, central differences, subaperture reduction and the
+ * column-major store including the zeros.
+ *   d_influence  DEVICE float32 [n_modes][ny][nx], 16-byte aligned
+ *   d_bbox       DEVICE int32 [n_modes][4] = (x0,y0,x1,y1) inclusive extent outside which the mode is
+ *                exactly zero (x1 < x0: the mode is identically zero), or NULL = dense modes.
+ *                A bbox that leaves out non-zero samples gives wrong results (not checked).
+ *   bbox_max_w/h HOST upper bounds of x1-x0+1 / y1-y0+1 over all modes, used only to size the
+ *                shared-memory tiles (<= 0: unknown).  Wrong bounds cost speed, never correctness.
+ *   affine       HOST [n_wfs]
+ *   mode         SYNIM_SLOPES_ND; SYNIM_SLOPES_GTILT returns SYNIM_ERR_UNSUPPORTED on this build
+ *   d_out        DEVICE float32, column-major, ld >= synim_num_rows(); every element of rows
+ *                [0, num_rows) of columns [0, n_modes) is written (padding rows are left untouched)
+ * Errors: INVALID_ARG (NULL, n_modes < 0, ld < rows, singular affine), ALIGNMENT, CUDA. */
+synim_status synim_interaction_matrix(const synim_geometry *geom, const float *d_influence, int32_t n_modes,
+                                      const int32_t *d_bbox, int32_t bbox_max_w, int32_t bbox_max_h,
+                                      const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out,
+                                      int64_t ld, void *stream);
+
+/* Tight non-zero extent of every mode of a cube (DEVICE in, DEVICE out int32 [n_modes][4]);
+ * an all-zero mode gets (0,0,-1,-1).  Asynchronous. */
+synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx,
+                                  int32_t *d_bbox, void *stream);
+/* Largest bbox width / height (HOST out); synchronises `stream`. */
+synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *max_w, int32_t *max_h,
+                               void *stream);
+
+/* Convenience wrapper with HOST buffers, for one-shot use and end-to-end timing: copies the cube
+ * (and bboxes, if given) to the device, runs synim_interaction_matrix, copies the IM back and
+ * synchronises.  h_out is column-major with ld = synim_num_rows().  Pinned host memory makes the
+ * copies asynchronous but is not required. */
+synim_status synim_interaction_matrix_host(const synim_geometry *geom, const float *h_influence, int32_t n_modes,
+                                           const int32_t *h_bbox, const synim_wfs_affine *affine,
+                                           synim_slope_mode mode, float *h_out, void *stream);
+
+void synim_destroy(synim_geometry *geom); /* NULL-safe; frees the internal device buffers */
+const char *synim_last_error(void);       /* thread-local, never NULL */
+int32_t synim_version(void);              /* major*1000 + minor */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SYNIM_H_ */

@@ -1,0 +1,428 @@
+// synim_api.cu -- host side of the C ABI declared in include/synim.h: argument checks, the static
+// geometry object (S0 of SURVEY.md sec. 8(a)), float64 composition / inversion of the per-sensor
+// affine maps, tile sizing, and the launches.  No compute happens here and there is no CPU path.
+#include "../../include/synim.h"
+#include "synim_device.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <vector>
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+synim_status fail(synim_status s, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return s;
+}
+
+synim_status cuda_fail(cudaError_t e, const char *what)
+{
+    if (e == cudaErrorMemoryAllocation) return fail(SYNIM_ERR_OUT_OF_MEMORY, "%s: %s", what, cudaGetErrorString(e));
+    return fail(SYNIM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+#define SYNIM_CUDA(call)                                       \
+    do {                                                       \
+        cudaError_t e_ = (call);                               \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);    \
+    } while (0)
+
+struct WfsHost {
+    int n_subap = 0, n_pix = 0, M = 0, n_valid = 0;
+    int row_x = 0, row_y = 0;
+    float *d_wmap = nullptr;
+    int *d_subap_row = nullptr;
+};
+
+}  // namespace
+
+struct synim_geometry {
+    int ny = 0, nx = 0, device = 0;
+    long long rows = 0;
+    std::vector<WfsHost> wfs;
+    // grow-only device workspace of synim_interaction_matrix_host / synim_bbox_extent
+    mutable std::mutex lock;
+    mutable float *ws_cube = nullptr;
+    mutable size_t ws_cube_bytes = 0;
+    mutable float *ws_out = nullptr;
+    mutable size_t ws_out_bytes = 0;
+    mutable int *ws_bbox = nullptr;
+    mutable size_t ws_bbox_bytes = 0;
+};
+
+namespace {
+
+synim_status check_device()
+{
+    int dev = 0, major = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    SYNIM_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10)
+        return fail(SYNIM_ERR_UNSUPPORTED_DEVICE, "device %d has compute capability %d.x; this library is sm_100a only",
+                    dev, major);
+    return SYNIM_OK;
+}
+
+int pow2_ceil(int v)
+{
+    int p = 1;
+    while (p < v) p <<= 1;
+    return p;
+}
+
+template <typename T>
+synim_status grow(T *&ptr, size_t &have, size_t want)
+{
+    if (want <= have) return SYNIM_OK;
+    if (ptr) cudaFree(ptr);
+    ptr = nullptr;
+    have = 0;
+    cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&ptr), want);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(workspace)");
+    have = want;
+    return SYNIM_OK;
+}
+
+// The absolute-index forward map and its inverse, in float64 (R1, R2).
+bool build_maps(const synim_wfs_affine &af, int M, int ny, int nx, double fwd[6], double inv[6])
+{
+    const double cw = (M - 1) / 2.0, cx = (nx - 1) / 2.0, cy = (ny - 1) / 2.0;
+    const double *a = af.a;
+    fwd[0] = a[0]; fwd[1] = a[1]; fwd[2] = a[2] + cx - cw * (a[0] + a[1]);
+    fwd[3] = a[3]; fwd[4] = a[4]; fwd[5] = a[5] + cy - cw * (a[3] + a[4]);
+    const double det = a[0] * a[4] - a[1] * a[3];
+    for (int k = 0; k < 6; ++k)
+        if (!std::isfinite(a[k])) return false;
+    if (!std::isfinite(af.slope_scale) || !(std::fabs(det) > 1e-300)) return false;
+    inv[0] = a[4] / det; inv[1] = -a[1] / det;
+    inv[3] = -a[3] / det; inv[4] = a[0] / det;
+    inv[2] = -(inv[0] * fwd[2] + inv[1] * fwd[5]);
+    inv[5] = -(inv[3] * fwd[2] + inv[4] * fwd[5]);
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *synim_last_error(void) { return g_err; }
+
+int32_t synim_version(void) { return SYNIM_VERSION_MAJOR * 1000 + SYNIM_VERSION_MINOR; }
+
+synim_status synim_compose_affine(const synim_wfs_physical *p, synim_wfs_affine *out)
+{
+    if (!p || !out) return fail(SYNIM_ERR_INVALID_ARG, "synim_compose_affine: NULL argument");
+    if (p->mag_x == 0.0 || p->mag_y == 0.0 || p->dm_mag == 0.0 || !(p->src_pixel_pitch_m > 0.0))
+        return fail(SYNIM_ERR_INVALID_ARG, "synim_compose_affine: zero magnification or non-positive pixel pitch");
+    const double deg = 3.14159265358979323846 / 180.0;
+    // 3x3 homogeneous matrices, multiplied right to left in the order of synim.h
+    struct H { double m[3][3]; };
+    auto mul = [](const H &A, const H &B) {
+        H C;
+        for (int i = 0; i < 3; ++i)
+            for (int j = 0; j < 3; ++j) C.m[i][j] = A.m[i][0] * B.m[0][j] + A.m[i][1] * B.m[1][j] + A.m[i][2] * B.m[2][j];
+        return C;
+    };
+    auto rotm = [](double t) { return H{{{std::cos(t), std::sin(t), 0}, {-std::sin(t), std::cos(t), 0}, {0, 0, 1}}}; };
+    auto scal = [](double sx, double sy) { return H{{{sx, 0, 0}, {0, sy, 0}, {0, 0, 1}}}; };
+    auto tran = [](double tx, double ty) { return H{{{1, 0, tx}, {0, 1, ty}, {0, 0, 1}}}; };
+    const double kappa = std::isinf(p->gs_range_m) ? 1.0 : 1.0 - p->dm_height_m / p->gs_range_m;
+    const double theta = p->gs_theta_arcsec * deg / 3600.0, az = p->gs_azimuth_deg * deg;
+    const double fx = p->dm_height_m * theta * std::cos(az) / p->src_pixel_pitch_m;
+    const double fy = p->dm_height_m * theta * std::sin(az) / p->src_pixel_pitch_m;
+    H T = scal(p->wfs_pitch_src_px, p->wfs_pitch_src_px);          // WFS pixel -> pupil-plane source pixels
+    T = mul(tran(-p->shift_x, -p->shift_y), T);                    // remove the WFS shift
+    T = mul(rotm(p->rot_deg * deg), T);                            // R(-rot)
+    T = mul(scal(1.0 / p->mag_x, 1.0 / p->mag_y), T);              // undo (anamorphic) magnification
+    T = mul(scal(kappa, kappa), T);                                // cone effect at the DM's altitude
+    T = mul(tran(fx - p->dm_shift_x, fy - p->dm_shift_y), T);      // footprint shift, DM shift
+    T = mul(rotm(p->dm_rot_deg * deg), T);                         // R(-dm_rot)
+    T = mul(scal(1.0 / p->dm_mag, 1.0 / p->dm_mag), T);
+    out->a[0] = T.m[0][0]; out->a[1] = T.m[0][1]; out->a[2] = T.m[0][2];
+    out->a[3] = T.m[1][0]; out->a[4] = T.m[1][1]; out->a[5] = T.m[1][2];
+    out->slope_scale = 1.0;
+    return SYNIM_OK;
+}
+
+void synim_destroy(synim_geometry *g)
+{
+    if (!g) return;
+    for (auto &w : g->wfs) {
+        if (w.d_wmap) cudaFree(w.d_wmap);
+        if (w.d_subap_row) cudaFree(w.d_subap_row);
+    }
+    if (g->ws_cube) cudaFree(g->ws_cube);
+    if (g->ws_out) cudaFree(g->ws_out);
+    if (g->ws_bbox) cudaFree(g->ws_bbox);
+    delete g;
+}
+
+synim_status synim_create_geometry(int32_t ny, int32_t nx, int32_t n_wfs, const synim_wfs_grid *grids, void *stream,
+                                   synim_geometry **out)
+{
+    if (!out) return fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: out is NULL");
+    *out = nullptr;
+    if (!grids || ny <= 0 || nx <= 0 || n_wfs < 1 || n_wfs > 64)
+        return fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: need grids, ny,nx > 0 and 1 <= n_wfs <= 64");
+    if (nx % 4 != 0) return fail(SYNIM_ERR_ALIGNMENT, "synim_create_geometry: nx = %d is not a multiple of 4", nx);
+    for (int w = 0; w < n_wfs; ++w) {
+        if (grids[w].n_subap < 1 || grids[w].n_pix < 1 || !grids[w].valid_mask || !grids[w].d_pupil)
+            return fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: sensor %d: bad n_subap / n_pix / NULL mask", w);
+        if ((long long)grids[w].n_subap * grids[w].n_pix > 32768)
+            return fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: sensor %d: more than 32768 pixels per side", w);
+    }
+    synim_status st = check_device();
+    if (st != SYNIM_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+
+    synim_geometry *g = new (std::nothrow) synim_geometry;
+    if (!g) return fail(SYNIM_ERR_OUT_OF_MEMORY, "synim_create_geometry: host allocation failed");
+    g->ny = ny; g->nx = nx;
+    cudaGetDevice(&g->device);
+    g->wfs.resize(n_wfs);
+
+    int *d_err = nullptr;
+    uint8_t *d_valid = nullptr;
+    size_t max_sub = 0;
+    for (int w = 0; w < n_wfs; ++w) max_sub = std::max(max_sub, (size_t)grids[w].n_subap * grids[w].n_subap);
+    auto cleanup = [&](synim_status r) {
+        if (d_err) cudaFree(d_err);
+        if (d_valid) cudaFree(d_valid);
+        if (r != SYNIM_OK) synim_destroy(g);
+        return r;
+    };
+    cudaError_t e;
+    if ((e = cudaMalloc(reinterpret_cast<void **>(&d_err), sizeof(int))) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMalloc"));
+    if ((e = cudaMalloc(reinterpret_cast<void **>(&d_valid), max_sub)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMalloc"));
+    if ((e = cudaMemsetAsync(d_err, 0, sizeof(int), s)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMemsetAsync"));
+
+    long long row = 0;
+    std::vector<int> rowmap;
+    std::vector<uint8_t> valid01;
+    for (int w = 0; w < n_wfs; ++w) {
+        WfsHost &h = g->wfs[w];
+        h.n_subap = grids[w].n_subap; h.n_pix = grids[w].n_pix; h.M = h.n_subap * h.n_pix;
+        const size_t ns = (size_t)h.n_subap * h.n_subap;
+        rowmap.assign(ns, -1);
+        valid01.assign(ns, 0);
+        int k = 0;
+        for (size_t q = 0; q < ns; ++q)
+            if (grids[w].valid_mask[q]) { rowmap[q] = k++; valid01[q] = 1; }
+        h.n_valid = k;
+        if (row + 2LL * k > 0x7fffffffLL) return cleanup(fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: more than 2^31 rows"));
+        h.row_x = (int)row; h.row_y = (int)row + k;
+        row += 2LL * k;
+        if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_wmap), sizeof(float) * (size_t)h.M * h.M)) != cudaSuccess)
+            return cleanup(cuda_fail(e, "cudaMalloc(wmap)"));
+        if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_subap_row), sizeof(int) * ns)) != cudaSuccess)
+            return cleanup(cuda_fail(e, "cudaMalloc(subap_row)"));
+        // pageable sources: these copies are staged by the runtime before the call returns
+        if ((e = cudaMemcpyAsync(h.d_subap_row, rowmap.data(), sizeof(int) * ns, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+            return cleanup(cuda_fail(e, "cudaMemcpyAsync(subap_row)"));
+        if ((e = cudaMemcpyAsync(d_valid, valid01.data(), ns, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+            return cleanup(cuda_fail(e, "cudaMemcpyAsync(valid)"));
+        if ((e = synim::launch_subap_weights(grids[w].d_pupil, d_valid, h.n_subap, h.n_pix, h.d_wmap, d_err, s)) != cudaSuccess)
+            return cleanup(cuda_fail(e, "subap_weights_kernel"));
+        // d_valid is reused by the next sensor: stream order keeps this safe
+    }
+    g->rows = row;
+    int herr = 0;
+    if ((e = cudaMemcpyAsync(&herr, d_err, sizeof(int), cudaMemcpyDeviceToHost, s)) != cudaSuccess)
+        return cleanup(cuda_fail(e, "cudaMemcpyAsync(err)"));
+    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaStreamSynchronize"));
+    if (herr) return cleanup(fail(SYNIM_ERR_EMPTY_SUBAP, "synim_create_geometry: a valid subaperture has zero summed pupil weight"));
+    *out = g;
+    return cleanup(SYNIM_OK);
+}
+
+int64_t synim_num_rows(const synim_geometry *g) { return g ? g->rows : -1; }
+
+int64_t synim_num_valid(const synim_geometry *g, int32_t w)
+{
+    return (g && w >= 0 && w < (int)g->wfs.size()) ? g->wfs[w].n_valid : -1;
+}
+
+int64_t synim_row_offset(const synim_geometry *g, int32_t w)
+{
+    return (g && w >= 0 && w < (int)g->wfs.size()) ? g->wfs[w].row_x : -1;
+}
+
+synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_influence, int32_t n_modes,
+                                      const int32_t *d_bbox, int32_t bbox_max_w, int32_t bbox_max_h,
+                                      const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out, int64_t ld,
+                                      void *stream)
+{
+    if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
+    if (mode == SYNIM_SLOPES_GTILT)
+        return fail(SYNIM_ERR_UNSUPPORTED, "synim_interaction_matrix: the G-tilt telescoping sum is not built on the GPU path");
+    if (mode != SYNIM_SLOPES_ND) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: unknown slope mode %d", (int)mode);
+    if (n_modes == 0) return SYNIM_OK;
+    if (!d_influence || !d_out) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL device buffer");
+    if (ld < g->rows) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: ld = %lld < rows = %lld", (long long)ld, g->rows);
+    if (reinterpret_cast<uintptr_t>(d_influence) % 16 != 0)
+        return fail(SYNIM_ERR_ALIGNMENT, "synim_interaction_matrix: influence cube is not 16-byte aligned");
+    if (reinterpret_cast<uintptr_t>(d_out) % 4 != 0 || (d_bbox && reinterpret_cast<uintptr_t>(d_bbox) % 16 != 0))
+        return fail(SYNIM_ERR_ALIGNMENT, "synim_interaction_matrix: output / bbox pointer misaligned");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int n_wfs = (int)g->wfs.size();
+    const bool dense = (d_bbox == nullptr);
+    const int ny = g->ny, nx = g->nx;
+
+    // ---- shared-memory tile sizing -------------------------------------------------------------
+    const int kPatchMax = 128, kTileMax = 96;
+    int bw = bbox_max_w, bh = bbox_max_h;
+    const bool hinted = !dense && bw > 0 && bh > 0 && bw + 2 <= kPatchMax && bh + 2 <= kPatchMax;
+    int patch_pitch, patch_h;
+    if (hinted) {
+        patch_pitch = (std::min(bw, nx) + 2 + 3) & ~3;
+        patch_h = std::min(bh, ny) + 2;
+    } else {
+        patch_pitch = 96;
+        patch_h = 96;
+    }
+
+    std::vector<synim::WfsDev> dev(n_wfs);
+    int tile_cap = 1;
+    for (int w = 0; w < n_wfs; ++w) {
+        const WfsHost &h = g->wfs[w];
+        synim::WfsDev &d = dev[w];
+        if (!build_maps(affine[w], h.M, ny, nx, d.fwd, d.inv))
+            return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: sensor %d: singular or non-finite affine", w);
+        d.wmap = h.d_wmap; d.subap_row = h.d_subap_row;
+        d.scale = (float)affine[w].slope_scale;
+        d.M = h.M; d.n_subap = h.n_subap; d.n_pix = h.n_pix; d.row_x = h.row_x; d.row_y = h.row_y;
+        d.group = std::min(32, pow2_ceil(h.n_pix));
+        d.pad_ = 0;
+        // tile edge when the whole support is one patch: large enough for the support's footprint
+        int tf = 64;
+        if (hinted) {
+            const double ew = (bw + 2) * std::fabs(d.inv[0]) + (bh + 2) * std::fabs(d.inv[1]);
+            const double eh = (bw + 2) * std::fabs(d.inv[3]) + (bh + 2) * std::fabs(d.inv[4]);
+            const double e = std::max(ew, eh);
+            tf = (e < 4096.0) ? (int)std::ceil(e) + 5 : kTileMax;
+        }
+        tf = std::max(8, std::min(tf, kTileMax));
+        tf = std::min(tf, h.M);
+        // tile edge when the patch is staged per tile: the source box of (t+2)^2 pixels plus 4 must fit
+        const double gx = std::fabs(d.fwd[0]) + std::fabs(d.fwd[1]), gy = std::fabs(d.fwd[3]) + std::fabs(d.fwd[4]);
+        const double lim_x = (patch_pitch - 5) / std::max(gx, 1e-12) - 1.0;
+        const double lim_y = (patch_h - 5) / std::max(gy, 1e-12) - 1.0;
+        int td = (int)std::floor(std::min({lim_x, lim_y, 64.0}));
+        td = std::max(1, std::min(td, h.M));
+        if (td >= h.n_pix) td -= td % h.n_pix;   // whole subapertures per tile when they fit
+        d.tile_fixed = tf; d.tile_dense = td;
+        tile_cap = std::max(tile_cap, std::max(tf, td));
+    }
+    const int phi_h = tile_cap + 2;
+    const int phi_pitch = (tile_cap + 2) | 1;   // odd pitch: rows of a subaperture fall in different banks
+    const size_t smem = sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)phi_pitch * phi_h);
+    if (smem > synim::max_dynamic_smem())
+        return fail(SYNIM_ERR_CUDA, "synim_interaction_matrix: %zu bytes of shared memory exceed the device limit", smem);
+
+    // ---- launches ------------------------------------------------------------------------------
+    if (dense) {
+        // several CTAs accumulate into one column: clear the rows first (one strided memset)
+        if (ld == g->rows) SYNIM_CUDA(cudaMemsetAsync(d_out, 0, sizeof(float) * (size_t)g->rows * n_modes, s));
+        else SYNIM_CUDA(cudaMemset2DAsync(d_out, sizeof(float) * (size_t)ld, 0, sizeof(float) * (size_t)g->rows, n_modes, s));
+    }
+    for (int w0 = 0; w0 < n_wfs; w0 += synim::kMaxWfsPerLaunch) {
+        const int nw = std::min(synim::kMaxWfsPerLaunch, n_wfs - w0);
+        synim::ImParams p;
+        std::memset(&p, 0, sizeof(p));
+        p.cube = d_influence; p.bbox = d_bbox; p.out = d_out; p.ld = ld;
+        p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
+        p.patch_pitch = patch_pitch; p.patch_h = patch_h; p.phi_pitch = phi_pitch; p.phi_h = phi_h;
+        for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
+        if (dense) {
+            p.zero_begin = 0; p.zero_count = 0;
+            p.chunks = 8;
+            p.jobs_per_mode = nw * p.chunks;
+        } else {
+            p.zero_begin = g->wfs[w0].row_x;
+            const WfsHost &last = g->wfs[w0 + nw - 1];
+            p.zero_count = last.row_x + 2 * last.n_valid - p.zero_begin;
+            p.chunks = 1;
+            p.jobs_per_mode = 1;
+        }
+        SYNIM_CUDA(synim::launch_interaction_matrix(p, smem, s));
+    }
+    return SYNIM_OK;
+}
+
+synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx, int32_t *d_bbox,
+                                  void *stream)
+{
+    if (n_modes < 0 || ny <= 0 || nx <= 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_compute_bboxes: bad sizes");
+    if (n_modes == 0) return SYNIM_OK;
+    if (!d_influence || !d_bbox) return fail(SYNIM_ERR_INVALID_ARG, "synim_compute_bboxes: NULL device buffer");
+    if (nx % 4 != 0 || reinterpret_cast<uintptr_t>(d_influence) % 16 != 0 || reinterpret_cast<uintptr_t>(d_bbox) % 16 != 0)
+        return fail(SYNIM_ERR_ALIGNMENT, "synim_compute_bboxes: need nx %% 4 == 0 and 16-byte aligned buffers");
+    SYNIM_CUDA(synim::launch_compute_bboxes(d_influence, n_modes, ny, nx, d_bbox, static_cast<cudaStream_t>(stream)));
+    return SYNIM_OK;
+}
+
+synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *max_w, int32_t *max_h, void *stream)
+{
+    if (!max_w || !max_h || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_bbox_extent: bad arguments");
+    *max_w = 0; *max_h = 0;
+    if (n_modes == 0) return SYNIM_OK;
+    if (!d_bbox) return fail(SYNIM_ERR_INVALID_ARG, "synim_bbox_extent: NULL device buffer");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int *d_wh = nullptr;
+    SYNIM_CUDA(cudaMalloc(reinterpret_cast<void **>(&d_wh), 2 * sizeof(int)));
+    int wh[2] = {0, 0};
+    cudaError_t e = synim::launch_bbox_extent(d_bbox, n_modes, d_wh, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(wh, d_wh, sizeof(wh), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d_wh);
+    if (e != cudaSuccess) return cuda_fail(e, "synim_bbox_extent");
+    *max_w = wh[0]; *max_h = wh[1];
+    return SYNIM_OK;
+}
+
+synim_status synim_interaction_matrix_host(const synim_geometry *g, const float *h_influence, int32_t n_modes,
+                                           const int32_t *h_bbox, const synim_wfs_affine *affine, synim_slope_mode mode,
+                                           float *h_out, void *stream)
+{
+    if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_host: bad arguments");
+    if (n_modes == 0) return SYNIM_OK;
+    if (!h_influence || !h_out) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_host: NULL host buffer");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    std::lock_guard<std::mutex> guard(g->lock);
+    const size_t cube_bytes = sizeof(float) * (size_t)n_modes * g->ny * g->nx;
+    const size_t out_bytes = sizeof(float) * (size_t)n_modes * (size_t)g->rows;
+    const size_t bbox_bytes = h_bbox ? sizeof(int) * 4 * (size_t)n_modes : 0;
+    synim_status st;
+    if ((st = grow(g->ws_cube, g->ws_cube_bytes, cube_bytes)) != SYNIM_OK) return st;
+    if ((st = grow(g->ws_out, g->ws_out_bytes, std::max<size_t>(out_bytes, 16))) != SYNIM_OK) return st;
+    if (h_bbox && (st = grow(g->ws_bbox, g->ws_bbox_bytes, bbox_bytes)) != SYNIM_OK) return st;
+    int bw = 0, bh = 0;
+    if (h_bbox) {
+        for (int m = 0; m < n_modes; ++m) {
+            bw = std::max(bw, h_bbox[4 * m + 2] - h_bbox[4 * m] + 1);
+            bh = std::max(bh, h_bbox[4 * m + 3] - h_bbox[4 * m + 1] + 1);
+        }
+        SYNIM_CUDA(cudaMemcpyAsync(g->ws_bbox, h_bbox, bbox_bytes, cudaMemcpyHostToDevice, s));
+    }
+    SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, h_influence, cube_bytes, cudaMemcpyHostToDevice, s));
+    st = synim_interaction_matrix(g, g->ws_cube, n_modes, h_bbox ? g->ws_bbox : nullptr, bw, bh, affine, mode, g->ws_out,
+                                  g->rows, s);
+    if (st != SYNIM_OK) return st;
+    SYNIM_CUDA(cudaMemcpyAsync(h_out, g->ws_out, out_bytes, cudaMemcpyDeviceToHost, s));
+    SYNIM_CUDA(cudaStreamSynchronize(s));
+    return SYNIM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,56 @@
+// synim_device.h -- structures shared by the host side of the C ABI (synim_api.cu) and the
+// sm_100a kernels (synim_kernels.cu).  Internal; the public interface is include/synim.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace synim {
+
+constexpr int kMaxWfsPerLaunch = 16;   // per-launch WFS batch (kernel-parameter space is 4 KB)
+constexpr int kThreads = 256;          // CTA size of the interaction-matrix kernel
+
+// One sensor as the kernel sees it.  All coordinates are ABSOLUTE pixel indices: WFS pixel (i, j)
+// (row, column) samples the source grid at
+//   col = fwd[0]*j + fwd[1]*i + fwd[2],   row = fwd[3]*j + fwd[4]*i + fwd[5]
+// (the centring terms (M-1)/2, (Nx-1)/2, (Ny-1)/2 of synim.h are folded into fwd[2], fwd[5] in
+// float64 on the host), and inv is the inverse map  j = inv[0]*col + inv[1]*row + inv[2],
+// i = inv[3]*col + inv[4]*row + inv[5].
+struct WfsDev {
+    double fwd[6];
+    double inv[6];
+    const float *wmap;       // [M][M]  0.5*P/W_S, 0 where the subaperture is invalid
+    const int *subap_row;    // [n_subap^2] index among the valid subapertures, -1 if invalid
+    float scale;             // slope_scale
+    int M, n_subap, n_pix;
+    int row_x, row_y;        // first row of the x / y slopes of this sensor inside a column
+    int tile_fixed;          // max edge (WFS pixels) of a D tile when the whole support is one patch
+    int tile_dense;          // max edge when the patch is re-staged per tile (its source box must fit)
+    int group;               // lanes that share one subaperture in the reduction (power of 2 <= 32)
+    int pad_;
+};
+
+struct ImParams {
+    const float *cube;       // [n_modes][ny][nx]
+    const int *bbox;         // [n_modes][4] or nullptr
+    float *out;              // column-major IM
+    long long ld;
+    int n_modes, ny, nx, n_wfs;
+    int patch_pitch, patch_h;   // shared-memory patch capacity, floats x rows
+    int phi_pitch, phi_h;       // shared-memory phi tile capacity including the 1-pixel halo
+    int zero_begin, zero_count; // rows [zero_begin, zero_begin+zero_count) of every column are zero-filled
+                                // by the mode's CTA before it accumulates (0: caller pre-zeroed)
+    int jobs_per_mode;          // 1: one CTA per mode walks every sensor; else n_wfs*chunks CTAs per mode
+    int chunks;                 // tile chunks per sensor when jobs_per_mode > 1
+    WfsDev wfs[kMaxWfsPerLaunch];
+};
+
+// launchers (synim_kernels.cu); all asynchronous on `stream`, return the launch status
+cudaError_t launch_interaction_matrix(const ImParams &p, size_t smem_bytes, cudaStream_t stream);
+cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
+                                 float *d_wmap, int *d_error_flag, cudaStream_t stream);
+cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox,
+                                  cudaStream_t stream);
+cudaError_t launch_bbox_extent(const int *d_bbox, int n_modes, int *d_wh, cudaStream_t stream);
+size_t max_dynamic_smem();  // opt-in limit of the current device (bytes)
+
+}  // namespace synim

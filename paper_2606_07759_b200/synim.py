@@ -1,0 +1,263 @@
+"""Thin ctypes binding of the C-ABI library (include/synim.h), same names without the prefix.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of ``libsynim.so``.
+PyTorch supplies device memory and streams.  There is no CPU fallback: if the library has not been
+built (``python -m paper_2606_07759_b200.build``) importing this module's functions raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsynim.so")
+
+OK, ERR_INVALID_ARG, ERR_ALIGNMENT, ERR_EMPTY_SUBAP = 0, -1, -2, -3
+ERR_UNSUPPORTED_DEVICE, ERR_OUT_OF_MEMORY, ERR_CUDA, ERR_UNSUPPORTED = -4, -5, -6, -7
+SLOPES_ND, SLOPES_GTILT = 0, 1
+
+#: every symbol include/synim.h declares
+EXPORTS = ("synim_compose_affine", "synim_create_geometry", "synim_num_rows", "synim_num_valid",
+           "synim_row_offset", "synim_interaction_matrix", "synim_compute_bboxes", "synim_bbox_extent",
+           "synim_interaction_matrix_host", "synim_destroy", "synim_last_error", "synim_version")
+
+PHYSICAL_FIELDS = ("shift_x", "shift_y", "rot_deg", "mag_x", "mag_y",
+                   "dm_shift_x", "dm_shift_y", "dm_rot_deg", "dm_mag",
+                   "dm_height_m", "gs_range_m", "gs_theta_arcsec", "gs_azimuth_deg",
+                   "src_pixel_pitch_m", "wfs_pitch_src_px")
+
+
+class WfsGrid(ctypes.Structure):
+    _fields_ = [("n_subap", ctypes.c_int32), ("n_pix", ctypes.c_int32),
+                ("valid_mask", ctypes.c_void_p), ("d_pupil", ctypes.c_void_p)]
+
+
+class WfsAffine(ctypes.Structure):
+    _fields_ = [("a", ctypes.c_double * 6), ("slope_scale", ctypes.c_double)]
+
+
+class WfsPhysical(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_double) for k in PHYSICAL_FIELDS]
+
+
+class SynimError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"synim status {status}: {text}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """The loaded library; raises if it was never built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_07759_b200.build`; "
+                               "there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        L.synim_compose_affine.restype = ctypes.c_int
+        L.synim_compose_affine.argtypes = [ctypes.POINTER(WfsPhysical), ctypes.POINTER(WfsAffine)]
+        L.synim_create_geometry.restype = ctypes.c_int
+        L.synim_create_geometry.argtypes = [i32, i32, i32, ctypes.POINTER(WfsGrid), vp, ctypes.POINTER(vp)]
+        for name in ("synim_num_rows",):
+            getattr(L, name).restype = i64
+            getattr(L, name).argtypes = [vp]
+        for name in ("synim_num_valid", "synim_row_offset"):
+            getattr(L, name).restype = i64
+            getattr(L, name).argtypes = [vp, i32]
+        L.synim_interaction_matrix.restype = ctypes.c_int
+        L.synim_interaction_matrix.argtypes = [vp, vp, i32, vp, i32, i32, ctypes.POINTER(WfsAffine), ctypes.c_int,
+                                               vp, i64, vp]
+        L.synim_compute_bboxes.restype = ctypes.c_int
+        L.synim_compute_bboxes.argtypes = [vp, i32, i32, i32, vp, vp]
+        L.synim_bbox_extent.restype = ctypes.c_int
+        L.synim_bbox_extent.argtypes = [vp, i32, ctypes.POINTER(i32), ctypes.POINTER(i32), vp]
+        L.synim_interaction_matrix_host.restype = ctypes.c_int
+        L.synim_interaction_matrix_host.argtypes = [vp, vp, i32, vp, ctypes.POINTER(WfsAffine), ctypes.c_int, vp, vp]
+        L.synim_destroy.restype = None
+        L.synim_destroy.argtypes = [vp]
+        L.synim_last_error.restype = ctypes.c_char_p
+        L.synim_last_error.argtypes = []
+        L.synim_version.restype = i32
+        L.synim_version.argtypes = []
+        _lib = L
+    return _lib
+
+
+def _check(status: int) -> None:
+    if status != OK:
+        raise SynimError(status, lib().synim_last_error().decode("utf-8", "replace"))
+
+
+def version() -> int:
+    return int(lib().synim_version())
+
+
+def last_error() -> str:
+    return lib().synim_last_error().decode("utf-8", "replace")
+
+
+def compose_affine(phys: dict) -> np.ndarray:
+    """Physical parameters (PHYSICAL_FIELDS) -> composite matrix a[6] (pure host call)."""
+    p = WfsPhysical(*[float(phys[k]) for k in PHYSICAL_FIELDS])
+    out = WfsAffine()
+    _check(lib().synim_compose_affine(ctypes.byref(p), ctypes.byref(out)))
+    return np.array(list(out.a), dtype=np.float64)
+
+
+def _affine_array(affines: Sequence[Sequence[float]], scales: Optional[Sequence[float]]):
+    n = len(affines)
+    arr = (WfsAffine * n)()
+    for k in range(n):
+        for q in range(6):
+            arr[k].a[q] = float(affines[k][q])
+        arr[k].slope_scale = 1.0 if scales is None else float(scales[k])
+    return arr
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+class Geometry:
+    """Owner of a ``synim_geometry*`` (synim_create_geometry / synim_destroy)."""
+
+    def __init__(self, ny: int, nx: int, wfs: Sequence, stream=None):
+        """``wfs``: objects with n_subap, n_pix, valid (uint8 [n_subap][n_subap], host) and pupil
+        (float32 [M][M]; a CUDA tensor, or a numpy array that is copied to the device here)."""
+        import torch
+        n = len(wfs)
+        grids = (WfsGrid * n)()
+        keep = []
+        for k, w in enumerate(wfs):
+            valid = np.ascontiguousarray(w.valid, dtype=np.uint8)
+            pupil = w.pupil
+            if not isinstance(pupil, torch.Tensor):
+                pupil = torch.from_numpy(np.ascontiguousarray(pupil, dtype=np.float32))
+            pupil = pupil.to(device="cuda", dtype=torch.float32).contiguous()
+            m = int(w.n_subap) * int(w.n_pix)
+            if tuple(pupil.shape) != (m, m) or valid.shape != (w.n_subap, w.n_subap):
+                raise ValueError(f"sensor {k}: pupil must be [{m}][{m}] and valid [{w.n_subap}][{w.n_subap}]")
+            keep.append((valid, pupil))
+            grids[k].n_subap, grids[k].n_pix = int(w.n_subap), int(w.n_pix)
+            grids[k].valid_mask = valid.ctypes.data
+            grids[k].d_pupil = pupil.data_ptr()
+        handle = ctypes.c_void_p()
+        _check(lib().synim_create_geometry(int(ny), int(nx), n, grids, _stream_ptr(stream), ctypes.byref(handle)))
+        self._h = handle
+        self.ny, self.nx, self.n_wfs = int(ny), int(nx), n
+        del keep   # synim_create_geometry synchronised the stream; the inputs are no longer read
+
+    @property
+    def num_rows(self) -> int:
+        return int(lib().synim_num_rows(self._h))
+
+    def num_valid(self, w: int) -> int:
+        return int(lib().synim_num_valid(self._h, int(w)))
+
+    def row_offset(self, w: int) -> int:
+        return int(lib().synim_row_offset(self._h, int(w)))
+
+    def destroy(self) -> None:
+        if getattr(self, "_h", None):
+            lib().synim_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def create_geometry(ny: int, nx: int, wfs: Sequence, stream=None) -> Geometry:
+    return Geometry(ny, nx, wfs, stream)
+
+
+def destroy(geom: Geometry) -> None:
+    geom.destroy()
+
+
+def num_rows(geom: Geometry) -> int:
+    return geom.num_rows
+
+
+def compute_bboxes(cube, stream=None):
+    """Tight non-zero extents of a CUDA float32 cube [n][ny][nx] -> CUDA int32 [n][4]."""
+    import torch
+    assert cube.is_cuda and cube.dtype == torch.float32 and cube.is_contiguous() and cube.dim() == 3
+    n, ny, nx = cube.shape
+    out = torch.empty((n, 4), dtype=torch.int32, device=cube.device)
+    _check(lib().synim_compute_bboxes(cube.data_ptr(), n, ny, nx, out.data_ptr(), _stream_ptr(stream)))
+    return out
+
+
+def bbox_extent(bbox, stream=None):
+    """(max width, max height) of CUDA int32 bboxes [n][4]; synchronises the stream."""
+    w, h = ctypes.c_int32(), ctypes.c_int32()
+    _check(lib().synim_bbox_extent(bbox.data_ptr(), int(bbox.shape[0]), ctypes.byref(w), ctypes.byref(h),
+                                   _stream_ptr(stream)))
+    return int(w.value), int(h.value)
+
+
+def interaction_matrix(geom: Geometry, cube, bbox, affines: Sequence[Sequence[float]],
+                       scales: Optional[Sequence[float]] = None, out=None, bbox_max=(0, 0),
+                       mode: int = SLOPES_ND, stream=None):
+    """synim_interaction_matrix on CUDA tensors.  Returns ``out`` viewed as [n_modes][ld] (row k of the
+    view is IM column k: the buffer is the column-major IM)."""
+    import torch
+    assert cube.is_cuda and cube.dtype == torch.float32 and cube.is_contiguous() and cube.dim() == 3
+    n = int(cube.shape[0])
+    if tuple(cube.shape[1:]) != (geom.ny, geom.nx):
+        raise ValueError("cube shape does not match the geometry's source grid")
+    if len(affines) != geom.n_wfs:
+        raise ValueError("one affine per sensor")
+    rows = geom.num_rows
+    if out is None:
+        out = torch.empty((n, rows), dtype=torch.float32, device=cube.device)
+    assert out.is_cuda and out.dtype == torch.float32 and out.dim() == 2 and out.stride(1) == 1
+    assert out.shape[0] >= n
+    ld = int(out.stride(0)) if out.shape[0] > 1 else int(out.shape[1])
+    bptr = None
+    if bbox is not None:
+        assert bbox.is_cuda and bbox.dtype == torch.int32 and bbox.is_contiguous() and tuple(bbox.shape) == (n, 4)
+        bptr = bbox.data_ptr()
+    arr = _affine_array(affines, scales)
+    _check(lib().synim_interaction_matrix(geom._h, cube.data_ptr(), n, bptr, int(bbox_max[0]), int(bbox_max[1]),
+                                          arr, int(mode), out.data_ptr(), ld, _stream_ptr(stream)))
+    return out
+
+
+def interaction_matrix_host(geom: Geometry, cube_host, bbox_host, affines: Sequence[Sequence[float]],
+                            scales: Optional[Sequence[float]] = None, out_host=None, mode: int = SLOPES_ND,
+                            stream=None):
+    """synim_interaction_matrix_host: HOST buffers in and out (torch CPU tensors, pinned or not, or
+    numpy arrays); copies and the final synchronisation happen inside the C call."""
+    import torch
+
+    def ptr(x):
+        return x.data_ptr() if isinstance(x, torch.Tensor) else x.ctypes.data
+
+    n = int(cube_host.shape[0])
+    rows = geom.num_rows
+    if out_host is None:
+        out_host = torch.empty((n, rows), dtype=torch.float32).pin_memory()
+    arr = _affine_array(affines, scales)
+    _check(lib().synim_interaction_matrix_host(geom._h, ptr(cube_host), n,
+                                               None if bbox_host is None else ptr(bbox_host),
+                                               arr, int(mode), ptr(out_host), _stream_ptr(stream)))
+    return out_host
+
+
+def affines_of(workload) -> list:
+    """Composite matrices of a ``workloads.Workload`` through the library's own helper."""
+    return [compose_affine(w.phys) for w in workload.wfs]

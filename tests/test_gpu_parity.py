@@ -1,0 +1,232 @@
+"""Parity of the CUDA path (through the C ABI) against the float64 oracle, on a B200.
+
+Tolerance (BASELINE.json north_star): per (mode, WFS) column relative L2 error <= 1e-5 and
+elementwise |err| <= 1e-5 * max|column| in float32; entries the oracle gives as exactly 0 must be
+exactly 0.  Every input is seeded and synthetic (paper_2606_07759_b200/workloads.py).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2606_07759_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def S():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the -m gpu tests need a CUDA device")
+    from paper_2606_07759_b200 import build, synim
+    build.build_library()
+    synim.lib()
+    return synim
+
+
+def gpu_im(S, wl, affines=None, scales=None, use_bbox=True, ld_pad=0, hint=True):
+    """IM of a workload through the C ABI -> numpy float32 [rows][n_modes]."""
+    import torch
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    cube = torch.from_numpy(wl.cube).cuda()
+    bbox, bmax = None, (0, 0)
+    if use_bbox and wl.bbox is not None:
+        bbox = torch.from_numpy(wl.bbox).cuda()
+        if hint:
+            bmax = S.bbox_extent(bbox)
+    rows = geom.num_rows
+    assert rows == wl.n_rows
+    out = torch.full((wl.n_modes, rows + ld_pad), float("nan"), dtype=torch.float32, device="cuda")
+    if affines is None:
+        affines = S.affines_of(wl)
+    if scales is None:
+        scales = [w.slope_scale for w in wl.wfs]
+    S.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax)
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    if ld_pad:
+        assert np.isnan(res[:, rows:]).all()      # padding rows are left untouched
+    geom.destroy()
+    return res[:, :rows].T.copy()
+
+
+def assert_parity(got, ref, wl, tol=TOL):
+    """got float32 [rows][n], ref float64 [rows][n]; checked per (mode, WFS) column."""
+    assert got.shape == ref.shape
+    assert np.isfinite(got).all()
+    r0 = 0
+    worst_l2 = worst_el = 0.0
+    for w in wl.wfs:
+        r1 = r0 + 2 * w.n_valid
+        g, r = got[r0:r1].astype(np.float64), ref[r0:r1]
+        err = np.abs(g - r)
+        cmax = np.abs(r).max(axis=0)
+        nrm = np.linalg.norm(r, axis=0)
+        live = cmax > 0
+        if live.any():
+            worst_l2 = max(worst_l2, float((np.linalg.norm(g - r, axis=0)[live] / nrm[live]).max()))
+            worst_el = max(worst_el, float((err.max(axis=0)[live] / cmax[live]).max()))
+        assert (g[:, ~live] == 0).all()
+        assert (g[r == 0] == 0).all(), "an entry the oracle gives as exactly 0 is not 0"
+        r0 = r1
+    assert worst_l2 <= tol and worst_el <= tol, (worst_l2, worst_el)
+    return worst_l2, worst_el
+
+
+def test_config1_scao_tiny_full(S):
+    wl = W.make_config(1)
+    assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
+
+
+def test_config1_with_padding_rows_scale_and_no_hint(S):
+    wl = W.make_config(1)
+    wl.wfs[0].slope_scale = 2.5
+    ref = O.interaction_matrix(wl)
+    assert_parity(gpu_im(S, wl, ld_pad=24), ref, wl)
+    assert_parity(gpu_im(S, wl, ld_pad=3), ref, wl)          # columns no longer 16-byte aligned
+    assert_parity(gpu_im(S, wl, hint=False), ref, wl)
+
+
+def test_config2_vlt_subset(S):
+    wl = W.make_config(2, max_modes=96)
+    assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
+
+
+def test_config3_elt_ground_six_rotated_lgs(S):
+    wl = W.make_config(3, max_modes=64)
+    assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
+
+
+def test_config4_altitude_dm_cone_footprint_and_giant_ngs_subaps(S):
+    wl = W.make_config(4, max_modes=48)
+    assert [w.n_pix for w in wl.wfs] == [7] * 6 + [238] * 3
+    assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
+
+
+def test_config5_dense_zernike_modes(S):
+    wl = W.make_config(5, max_modes=10)
+    assert wl.bbox is None
+    assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
+
+
+def test_dense_path_on_zonal_cube_equals_bbox_path(S):
+    """bbox = NULL must give the same matrix as the tile-skipping path (skipping is exact, R15)."""
+    wl = W.make_config(1, max_modes=24)
+    ref = O.interaction_matrix(wl)
+    assert_parity(gpu_im(S, wl, use_bbox=False), ref, wl)
+
+
+def test_identity_transform_is_exact_on_integer_data(S):
+    """Identity map: phi == input bit for bit, so slopes of an integer-valued screen with P = 1
+    are exactly representable sums: the GPU must match the oracle to the last bit."""
+    rng = np.random.default_rng(31)
+    n_subap, n_pix = 6, 8
+    m = n_subap * n_pix
+    cube = rng.integers(-8, 9, size=(5, m, m)).astype(np.float32)
+    w = W.WfsInput(n_subap, n_pix, np.ones((m, m), np.float32), np.ones((n_subap, n_subap), np.uint8), W.physical())
+    wl = W.Workload("identity", 0, m, m, cube, None, [w])
+    got = gpu_im(S, wl)
+    ref = O.interaction_matrix(wl)
+    assert np.array_equal(got.astype(np.float64), ref)
+
+
+def test_tilt_and_quadratic_closed_forms_on_the_gpu(S):
+    """The oracle's closed-form pins, applied directly to the CUDA path."""
+    n = 96
+    yy, xx = np.mgrid[0:n, 0:n].astype(np.float64)
+    xs, ys = xx - (n - 1) / 2.0, yy - (n - 1) / 2.0
+    ta, tb = 0.375, -0.5
+    cube = np.stack([ta * xs + tb * ys, xs ** 2 / 64.0]).astype(np.float32)
+    rng = np.random.default_rng(32)
+    n_subap, n_pix = 6, 5
+    pupil = rng.uniform(0.1, 1.0, (30, 30)).astype(np.float32)
+    w = W.WfsInput(n_subap, n_pix, pupil, np.ones((6, 6), np.uint8), W.physical(), slope_scale=1.5)
+    wl = W.Workload("closed forms", 0, n, n, cube, None, [w])
+    t = math.radians(27.0)
+    a = [math.cos(t) / 1.07, math.sin(t) / 1.07, 0.31, -math.sin(t) / 1.07, math.cos(t) / 1.07, -0.44]
+    got = gpu_im(S, wl, affines=[a])
+    assert np.allclose(got[:36, 0], 1.5 * (ta * a[0] + tb * a[3]), rtol=0, atol=1e-5)
+    assert np.allclose(got[36:, 0], 1.5 * (ta * a[1] + tb * a[4]), rtol=0, atol=1e-5)
+    got = gpu_im(S, wl, affines=[[1, 0, 0.25, 0, 1, -1.5]])
+    p = pupil.astype(np.float64).reshape(6, 5, 6, 5)
+    xw = (np.arange(30) - 14.5).reshape(1, 1, 6, 5)
+    xbar = (p * xw).sum(axis=(1, 3)) / p.sum(axis=(1, 3))
+    assert np.allclose(got[:36, 1], 1.5 * 2 * (xbar.ravel() + 0.25) / 64.0, rtol=0, atol=1e-5)
+    assert np.allclose(got[36:, 1], 0.0, atol=1e-5)
+
+
+def test_empty_and_degenerate_inputs(S):
+    import torch
+    wl = W.make_config(1, max_modes=6)
+    wl.cube[2] = 0.0                               # an identically-zero mode
+    wl.bbox[2] = (0, 0, -1, -1)
+    wl.bbox[4] = (0, 0, wl.nx - 1, wl.ny - 1)      # a loose, full-grid bbox is still correct
+    ref = O.interaction_matrix(wl)
+    got = gpu_im(S, wl, hint=False)
+    assert (got[:, 2] == 0).all()
+    assert_parity(got, ref, wl)
+    # n_modes = 0 is a no-op
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    empty = torch.empty((0, wl.ny, wl.nx), dtype=torch.float32, device="cuda")
+    out = S.interaction_matrix(geom, empty, None, S.affines_of(wl))
+    assert out.shape == (0, geom.num_rows)
+    # singular affine and a too-small ld are argument errors
+    cube = torch.from_numpy(wl.cube).cuda()
+    with pytest.raises(S.SynimError) as e:
+        S.interaction_matrix(geom, cube, None, [[1, 2, 0, 2, 4, 0]])
+    assert e.value.status == S.ERR_INVALID_ARG
+    with pytest.raises(S.SynimError) as e:
+        S.interaction_matrix(geom, cube, None, S.affines_of(wl), mode=S.SLOPES_GTILT)
+    assert e.value.status == S.ERR_UNSUPPORTED
+    small = torch.empty((wl.n_modes, geom.num_rows - 1), dtype=torch.float32, device="cuda")
+    assert S.lib().synim_interaction_matrix(geom._h, cube.data_ptr(), wl.n_modes, None, 0, 0,
+                                            S._affine_array(S.affines_of(wl), None), 0, small.data_ptr(),
+                                            geom.num_rows - 1, None) == S.ERR_INVALID_ARG
+    geom.destroy()
+    # a valid subaperture without light is refused at geometry creation
+    dark = W.WfsInput(2, 4, np.zeros((8, 8), np.float32), np.ones((2, 2), np.uint8), W.physical())
+    with pytest.raises(S.SynimError) as e:
+        S.create_geometry(8, 8, [dark])
+    assert e.value.status == S.ERR_EMPTY_SUBAP
+
+
+def test_wfs_looking_past_the_source_grid_and_strong_magnification(S):
+    """Footprints that overrun the grid (R4), a demagnified and an anamorphic sensor, partial pupil."""
+    rng = np.random.default_rng(33)
+    ny, nx = 72, 88
+    cube = W.random_smooth_cube(6, ny, nx, 34)
+    pup = W.make_pupil(60, 60.0, 0.2)
+    sensors = []
+    for phys in (W.physical(shift_x=20.0, shift_y=-17.5, rot_deg=33.0),
+                 W.physical(mag_x=0.55, mag_y=0.6, rot_deg=-75.0),
+                 W.physical(mag_x=1.7, mag_y=1.5, shift_x=3.3, rot_deg=140.0)):
+        sensors.append(W.WfsInput(10, 6, pup, W.valid_subaps(pup, 10, 6), phys))
+    wl = W.Workload("overrun", 0, ny, nx, cube, None, sensors)
+    ref = O.interaction_matrix(wl)
+    assert_parity(gpu_im(S, wl), ref, wl)
+    wl.bbox = W.tight_bboxes(cube)
+    assert_parity(gpu_im(S, wl), ref, wl)
+    assert_parity(gpu_im(S, wl, hint=False), ref, wl)
+
+
+def test_compute_bboxes_matches_the_generator(S):
+    import torch
+    wl = W.make_config(2, max_modes=40)
+    wl.cube[7] = 0
+    got = S.compute_bboxes(torch.from_numpy(wl.cube).cuda())
+    exp = W.tight_bboxes(wl.cube)
+    assert np.array_equal(got.cpu().numpy(), exp)
+    assert S.bbox_extent(got) == (int((exp[:, 2] - exp[:, 0] + 1).max()), int((exp[:, 3] - exp[:, 1] + 1).max()))
+
+
+def test_host_buffer_entry_point(S):
+    import torch
+    wl = W.make_config(1)
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    out = S.interaction_matrix_host(geom, torch.from_numpy(wl.cube).pin_memory(), wl.bbox, S.affines_of(wl))
+    assert_parity(out.numpy().T.copy(), O.interaction_matrix(wl), wl)
+    geom.destroy()

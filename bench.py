@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- IM columns/s of the synthetic Shack-Hartmann interaction matrix on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (S1-S4 of SURVEY.md sec. 8(a)) over one synthetic
+workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators x 6 LGS WFS =
+30,390 columns).  One JSON line is printed by rank 0.
+
+  value     columns/s, inputs resident in HBM, CUDA events around K back-to-back calls
+  e2e       columns/s through synim_interaction_matrix_host: pinned HOST cube/bboxes in, HOST IM out,
+            copies inside the timed region
+  roofline  algorithmic bytes (IF bytes that must be read + IM bytes written) / average
+            kernel time (one CUDA-event pair per step) against the measured HBM copy bandwidth
+  cpu_baseline  the float64 oracle, as it stands, on the host cores, on a bounded sample of modes
+
+--impl reference times the oracle only (rank 0; other ranks exit).  N > 1: every rank holds its own
+workload of the same shape (independent problems, no data-path collective): weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "IM columns/s (actuator x WFS)"
+UNIT = "columns/s"
+FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+def algorithmic_bytes(wl) -> dict:
+    """IF bytes that must be read once (32-byte sectors of each bbox row; the whole mode when dense)
+    plus IM bytes written."""
+    if wl.bbox is not None:
+        b = wl.bbox.astype(np.int64)
+        w = np.maximum(b[:, 2] - b[:, 0] + 1, 0)
+        h = np.maximum(b[:, 3] - b[:, 1] + 1, 0)
+        read = int((h * ((w * 4 + 31) // 32) * 32).sum())
+    else:
+        read = int(wl.n_modes) * wl.ny * wl.nx * 4
+    write = int(wl.n_rows) * int(wl.n_modes) * 4
+    return {"read": read, "write": write, "total": read + write}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth, burst)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def profile_traffic(cfg: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu summary."""
+    p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    try:
+        best = None
+        for line in open(p):
+            f = [x.strip() for x in line.split(",")]
+            if f and f[0] == f"cfg{cfg}":
+                best = float(f[1]) + float(f[2])      # the last matching line is the newest round
+        return best
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.1] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except Exception:
+                continue
+            for nme, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_throughput(wl, target_s: float, n_threads: int = 0):
+    """Time the oracle (as it stands, OpenMP over modes) on a seeded sample of modes sized for about
+    ``target_s`` seconds.  Returns (columns/s, cores, description)."""
+    from oracle import oracle as O
+    cores = O.num_threads() if n_threads <= 0 else n_threads
+    rng = np.random.default_rng(7759)
+    probe = np.sort(rng.choice(wl.n_modes, size=min(wl.n_modes, max(cores, 8)), replace=False))
+    t0 = time.perf_counter()
+    O.interaction_matrix(wl, modes=probe, n_threads=n_threads)
+    dt = time.perf_counter() - t0
+    n = int(min(wl.n_modes, max(len(probe), round(len(probe) * target_s / max(dt, 1e-6)))))
+    sel = np.sort(rng.choice(wl.n_modes, size=n, replace=False))
+    t0 = time.perf_counter()
+    O.interaction_matrix(wl, modes=sel, n_threads=n_threads)
+    dt = time.perf_counter() - t0
+    cols = n * len(wl.wfs)
+    return cols / dt, cores, f"{n} of {wl.n_modes} modes (seeded draw) x {len(wl.wfs)} WFS = {cols} columns in {dt:.1f} s"
+
+
+def config_dict(wl, extra=None):
+    d = {"workload": f"BASELINE.json configs[{wl.cfg - 1}]: {wl.name}", "n_modes": wl.n_modes, "n_wfs": len(wl.wfs),
+         "columns": wl.n_columns, "im_rows": wl.n_rows, "grid": [wl.ny, wl.nx],
+         "l2": "no explicit flush: every step streams the whole IM (larger than the 126 MB L2) through L2"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def run_reference(args, rank: int):
+    if rank != 0:
+        return
+    from paper_2606_07759_b200 import workloads
+    wl = workloads.make_config(args.config)
+    per_step_s = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    vals, desc, cores = [], "", 0
+    for k in range(args.warmup + args.steps):
+        v, cores, desc = oracle_throughput(wl, per_step_s)
+        if k >= args.warmup:
+            vals.append(v)
+    value = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wl.n_columns / value,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(wl, {"note": "float64 CPU oracle; each step is a bounded sample, ms_per_step extrapolated"}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    from paper_2606_07759_b200 import build, sharding, synim, workloads
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        build.build_library()
+    if dist is not None:
+        dist.barrier()
+    synim.lib()
+    warmup = max(args.warmup, 3)
+
+    # every rank: its own workload of the same shape (independent problems -> weak scaling)
+    wl = workloads.make_config(args.config)
+    affines = synim.affines_of(wl)
+    scales = [w.slope_scale for w in wl.wfs]
+    geom = synim.create_geometry(wl.ny, wl.nx, wl.wfs)
+    cube = torch.from_numpy(wl.cube).cuda()
+    bbox, bmax = None, (0, 0)
+    if wl.bbox is not None:
+        bbox = synim.compute_bboxes(cube)
+        bmax = synim.bbox_extent(bbox)
+    out = torch.empty((wl.n_modes, geom.num_rows), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        synim.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax, stream=stream)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t_wall0 = time.time()
+    ev[0].record(stream)
+    for k in range(args.steps):
+        step()
+        ev[k + 1].record(stream)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t_wall1 = time.time()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_step = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)])
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+
+    # spot-check the timed launch configuration against the oracle on sampled columns (rank 0)
+    parity = None
+    if rank == 0:
+        from oracle import oracle as O
+        rng = np.random.default_rng(7759 + 100)
+        sel = np.sort(rng.choice(wl.n_modes, size=min(8, wl.n_modes), replace=False))
+        ref = O.interaction_matrix(wl, modes=sel)
+        got = out[torch.from_numpy(sel).cuda()].cpu().numpy().T.astype(np.float64)
+        cmax = np.abs(ref).max(axis=0)
+        parity = {"sampled_modes": int(len(sel)),
+                  "max_rel_l2": float((np.linalg.norm(got - ref, axis=0) / np.linalg.norm(ref, axis=0)).max()),
+                  "max_elementwise": float((np.abs(got - ref).max(axis=0) / cmax).max())}
+
+    # end to end through the HOST-buffer entry point (pinned host memory, copies inside the timing)
+    e2e = None
+    if not args.no_e2e:
+        h_cube = torch.from_numpy(wl.cube).pin_memory()
+        h_bbox = None if wl.bbox is None else torch.from_numpy(wl.bbox).pin_memory()
+        h_out = torch.empty((wl.n_modes, geom.num_rows), dtype=torch.float32).pin_memory()
+        synim.interaction_matrix_host(geom, h_cube, h_bbox, affines, scales, out_host=h_out, stream=stream)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            synim.interaction_matrix_host(geom, h_cube, h_bbox, affines, scales, out_host=h_out, stream=stream)
+        torch.cuda.synchronize()
+        e2e_ms = 1e3 * (time.perf_counter() - t0) / args.e2e_steps
+        h2d = h_cube.numel() * 4 + (0 if h_bbox is None else h_bbox.numel() * 4)
+        d2h = h_out.numel() * 4
+        e2e = (e2e_ms, h2d, d2h)
+
+    times = torch.tensor([total_ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(times[0]), float(times[1])
+    plan = sharding.weak_scaling_plan(wl.n_columns, world)
+
+    if rank == 0:
+        ms_per_step = total_ms / args.steps
+        value = plan["total_units"] / (ms_per_step * 1e-3)
+        ab = algorithmic_bytes(wl)
+        peak, peak_src = measured_peak()
+        kernel_ms = float(per_step.mean())
+        achieved = ab["total"] / (kernel_ms * 1e-3) / 1e9
+        traffic = profile_traffic(args.config)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": config_dict(wl, {"parallelism": f"{world} independent workloads, one per GPU, no collective",
+                                           "per_step_ms_min_med_max": [float(per_step.min()), float(np.median(per_step)),
+                                                                       float(per_step.max())]}),
+                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                             "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                             "algorithmic_bytes": ab, "kernel": "synim_im_kernel", "kernel_ms": kernel_ms},
+                "clocks": clocks, "gpu_launches": args.steps * (1 if wl.bbox is not None else 1),
+                "parity_spot_check": parity}
+        if e2e:
+            line["e2e"] = {"value": plan["total_units"] / (e2e_ms * 1e-3), "unit": UNIT,
+                           "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2], "ms_per_step": e2e_ms,
+                           "api": "synim_interaction_matrix_host (pinned host buffers)"}
+        if world == 1 and not args.no_cpu_baseline:
+            v, cores, desc = oracle_throughput(wl, 10.0)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        print(json.dumps(line), flush=True)
+    geom.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

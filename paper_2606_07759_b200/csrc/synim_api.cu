@@ -4,6 +4,8 @@
 #include "../../include/synim.h"
 #include "synim_device.h"
 
+#include <cuda.h>   // CUtensorMap and its enums; cuTensorMapEncodeTiled is fetched through the runtime
+
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
@@ -111,6 +113,35 @@ bool build_maps(const synim_wfs_affine &af, int M, int ny, int nx, double fwd[6]
     inv[2] = -(inv[0] * fwd[2] + inv[1] * fwd[5]);
     inv[5] = -(inv[3] * fwd[2] + inv[4] * fwd[5]);
     return true;
+}
+
+// TMA descriptor over the cube [n_modes][ny][nx] with box {box_w, box_h, 1}; out-of-range elements read
+// as zero.  The driver entry point comes from the runtime, so libcuda is never linked.
+synim_status encode_cube_map(const float *d_cube, int n_modes, int ny, int nx, int box_w, int box_h, CUtensorMap *out)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn fn = nullptr;
+    if (!fn) {
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q);
+        if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !sym)
+            return fail(SYNIM_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+        fn = reinterpret_cast<encode_fn>(sym);
+    }
+    if (box_w < 4 || box_w > 256 || box_h < 1 || box_h > 256 || box_w % 4 != 0)
+        return fail(SYNIM_ERR_INVALID_ARG, "internal: TMA box %d x %d out of range", box_w, box_h);
+    const cuuint64_t dims[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)n_modes};
+    const cuuint64_t strides[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * (cuuint64_t)ny * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)box_w, (cuuint32_t)box_h, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(d_cube), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(SYNIM_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    return SYNIM_OK;
 }
 
 }  // namespace
@@ -288,6 +319,9 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     if (hinted) {
         patch_pitch = (std::min(bw, nx) + 2 + 3) & ~3;
         patch_h = std::min(bh, ny) + 2;
+    } else if (!dense) {
+        patch_pitch = 64;   // unknown support size: 62 x 62 pieces (larger supports are split, by linearity)
+        patch_h = 64;
     } else {
         patch_pitch = 96;
         patch_h = 96;
@@ -327,7 +361,13 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     }
     const int phi_h = tile_cap + 2;
     const int phi_pitch = (tile_cap + 2) | 1;   // odd pitch: rows of a subaperture fall in different banks
-    const size_t smem = sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)phi_pitch * phi_h);
+    const size_t smem = dense ? sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)phi_pitch * phi_h)
+                              : sizeof(float) * (size_t)patch_pitch * patch_h;
+    CUtensorMap tmap;
+    if (!dense) {
+        synim_status st = encode_cube_map(d_influence, n_modes, ny, nx, patch_pitch, patch_h, &tmap);
+        if (st != SYNIM_OK) return st;
+    }
     if (smem > synim::max_dynamic_smem())
         return fail(SYNIM_ERR_CUDA, "synim_interaction_matrix: %zu bytes of shared memory exceed the device limit", smem);
 
@@ -356,7 +396,8 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
             p.chunks = 1;
             p.jobs_per_mode = 1;
         }
-        SYNIM_CUDA(synim::launch_interaction_matrix(p, smem, s));
+        if (dense) SYNIM_CUDA(synim::launch_interaction_matrix(p, smem, s));
+        else SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));
     }
     return SYNIM_OK;
 }

@@ -46,6 +46,9 @@ struct ImParams {
 
 // launchers (synim_kernels.cu); all asynchronous on `stream`, return the launch status
 cudaError_t launch_interaction_matrix(const ImParams &p, size_t smem_bytes, cudaStream_t stream);
+// compact-support path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
+// {patch_pitch, patch_h, 1}
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
                                  float *d_wmap, int *d_error_flag, cudaStream_t stream);
 cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox,

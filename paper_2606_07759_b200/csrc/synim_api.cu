@@ -314,13 +314,13 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     // ---- shared-memory tile sizing -------------------------------------------------------------
     const int kPatchMax = 128, kTileMax = 96;
     int bw = bbox_max_w, bh = bbox_max_h;
-    const bool hinted = !dense && bw > 0 && bh > 0 && bw + 2 <= kPatchMax && bh + 2 <= kPatchMax;
+    const bool hinted = !dense && bw > 0 && bh > 0 && bw + 5 <= kPatchMax && bh + 2 <= kPatchMax;
     int patch_pitch, patch_h;
     if (hinted) {
-        patch_pitch = (std::min(bw, nx) + 2 + 3) & ~3;
+        patch_pitch = (std::min(bw, nx) + 5 + 3) & ~3;   // ring + up to 3 columns of TMA alignment slack
         patch_h = std::min(bh, ny) + 2;
     } else if (!dense) {
-        patch_pitch = 64;   // unknown support size: 62 x 62 pieces (larger supports are split, by linearity)
+        patch_pitch = 68;   // unknown support size: 63 x 62 pieces (larger supports are split, by linearity)
         patch_h = 64;
     } else {
         patch_pitch = 96;

@@ -220,7 +220,8 @@ __global__ void __launch_bounds__(kStripThreads) synim_strip_kernel(const __grid
     const bool empty = bx1 < bx0 || by1 < by0;
 
     // pieces of the support that fit the staged box (one piece unless the bbox hint was too small)
-    const int cap_w = p.patch_pitch - 2, cap_h = p.patch_h - 2;
+    // (the box must start on a 16-byte boundary of the source row: up to 3 columns of slack on the left)
+    const int cap_w = p.patch_pitch - 5, cap_h = p.patch_h - 2;
     const int npcx = empty ? 0 : (bx1 - bx0 + cap_w) / cap_w, npcy = empty ? 0 : (by1 - by0 + cap_h) / cap_h;
     const int npieces = npcx * npcy;
     const uint32_t box_bytes = (uint32_t)(p.patch_pitch * p.patch_h) * 4u;
@@ -228,8 +229,9 @@ __global__ void __launch_bounds__(kStripThreads) synim_strip_kernel(const __grid
     if (tid == 0 && npieces > 0) {
         mbar_init(&bar, 1);
         fence_barrier_init();
+        fence_proxy_async();
         mbar_expect_tx(&bar, box_bytes);
-        tma_load_box(patch, &tmap, &bar, bx0 - 1, by0 - 1, mode);
+        tma_load_box(patch, &tmap, &bar, (bx0 - 1) & ~3, by0 - 1, mode);
     }
     if (p.zero_count > 0) zero_fill<kStripThreads>(colp + p.zero_begin, p.zero_count);
     __syncthreads();   // barrier initialised; this CTA's zeros are ordered before its accumulations
@@ -240,13 +242,17 @@ __global__ void __launch_bounds__(kStripThreads) synim_strip_kernel(const __grid
         const int qx0 = bx0 + pcx * cap_w, qx1 = min(qx0 + cap_w - 1, bx1);
         const int qy0 = by0 + pcy * cap_h, qy1 = min(qy0 + cap_h - 1, by1);
         PatchBox pa;
-        pa.x0 = qx0 - 1; pa.y0 = qy0 - 1; pa.w = qx1 - qx0 + 3; pa.h = qy1 - qy0 + 3;
+        pa.x0 = (qx0 - 1) & ~3; pa.y0 = qy0 - 1; pa.w = qx1 + 2 - pa.x0; pa.h = qy1 - qy0 + 3;
+        const int slack = qx0 - 1 - pa.x0;   // columns 0..slack are left of the piece
         mbar_wait(&bar, parity);
         parity ^= 1u;
         if (npieces > 1) {
             // by linearity a piece is its own mode: zero outside its box, so clear the ring just staged
             for (int e = tid; e < pa.w; e += kStripThreads) { patch[e] = 0.0f; patch[(pa.h - 1) * p.patch_pitch + e] = 0.0f; }
-            for (int e = tid; e < pa.h; e += kStripThreads) { patch[e * p.patch_pitch] = 0.0f; patch[e * p.patch_pitch + pa.w - 1] = 0.0f; }
+            for (int e = tid; e < pa.h; e += kStripThreads) {
+                for (int c = 0; c <= slack; ++c) patch[e * p.patch_pitch + c] = 0.0f;
+                patch[e * p.patch_pitch + pa.w - 1] = 0.0f;
+            }
             __syncthreads();
         }
 
@@ -292,7 +298,7 @@ __global__ void __launch_bounds__(kStripThreads) synim_strip_kernel(const __grid
                 const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
                 fence_proxy_async();
                 mbar_expect_tx(&bar, box_bytes);
-                tma_load_box(patch, &tmap, &bar, bx0 + nx_ * cap_w - 1, by0 + ny_ * cap_h - 1, mode);
+                tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
             }
         }
     }

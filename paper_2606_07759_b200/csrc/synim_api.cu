@@ -11,6 +11,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <mutex>
 #include <new>
 #include <vector>
@@ -255,8 +256,11 @@ synim_status synim_create_geometry(int32_t ny, int32_t nx, int32_t n_wfs, const 
         if (row + 2LL * k > 0x7fffffffLL) return cleanup(fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: more than 2^31 rows"));
         h.row_x = (int)row; h.row_y = (int)row + k;
         row += 2LL * k;
-        if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_wmap), sizeof(float) * (size_t)h.M * h.M)) != cudaSuccess)
+        // rows of zeros below the map: the strip kernel's halo lanes and row look-ahead read them
+        const size_t wmap_bytes = sizeof(float) * (size_t)(h.M + synim::kWmapPadRows) * h.M;
+        if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_wmap), wmap_bytes)) != cudaSuccess)
             return cleanup(cuda_fail(e, "cudaMalloc(wmap)"));
+        if ((e = cudaMemsetAsync(h.d_wmap, 0, wmap_bytes, s)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMemsetAsync(wmap)"));
         if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_subap_row), sizeof(int) * ns)) != cudaSuccess)
             return cleanup(cuda_fail(e, "cudaMalloc(subap_row)"));
         // pageable sources: these copies are staged by the runtime before the call returns
@@ -317,8 +321,8 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     const bool hinted = !dense && bw > 0 && bh > 0 && bw + 5 <= kPatchMax && bh + 2 <= kPatchMax;
     int patch_pitch, patch_h;
     if (hinted) {
-        patch_pitch = (std::min(bw, nx) + 5 + 3) & ~3;   // ring + up to 3 columns of TMA alignment slack
-        patch_h = std::min(bh, ny) + 2;
+        patch_pitch = (std::min(bw, nx) + 5 + 3) & ~3;   // <= 3 columns of TMA alignment slack, ring, support, ring
+        patch_h = std::min(bh, ny) + 2;                  // ring, support, ring
     } else if (!dense) {
         patch_pitch = 68;   // unknown support size: 63 x 62 pieces (larger supports are split, by linearity)
         patch_h = 64;
@@ -338,7 +342,7 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         d.scale = (float)affine[w].slope_scale;
         d.M = h.M; d.n_subap = h.n_subap; d.n_pix = h.n_pix; d.row_x = h.row_x; d.row_y = h.row_y;
         d.group = std::min(32, pow2_ceil(h.n_pix));
-        d.pad_ = 0;
+        d.pad_ = 0; d.tab_off = 0; d.tab_cap = 0;
         // tile edge when the whole support is one patch: large enough for the support's footprint
         int tf = 64;
         if (hinted) {
@@ -361,8 +365,43 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     }
     const int phi_h = tile_cap + 2;
     const int phi_pitch = (tile_cap + 2) | 1;   // odd pitch: rows of a subaperture fall in different banks
+    // strip kernel: one float4 bilinear cell per pixel pair of (piece + ring) behind the raw TMA box
+    const int cell_pitch = patch_pitch - 5 + 1, cell_h = patch_h - 2 + 1;
+    // strip kernel: per sensor a table of (x, y) partial slopes over the window of subapertures one
+    // piece's footprint can span (the kernel derives the window from the same bounds and traps if it
+    // ever needed more)
+    int tab_floats_max = 0;
+    if (!dense) {
+        const int cap_w = patch_pitch - 5, cap_h = patch_h - 2;
+        for (int w0 = 0; w0 < n_wfs; w0 += synim::kMaxWfsPerLaunch) {
+            int off = 0;
+            for (int w = w0; w < std::min(n_wfs, w0 + synim::kMaxWfsPerLaunch); ++w) {
+                synim::WfsDev &d = dev[w];
+                const double ej = (cap_w + 2) * std::fabs(d.inv[0]) + (cap_h + 2) * std::fabs(d.inv[1]);
+                const double ei = (cap_w + 2) * std::fabs(d.inv[3]) + (cap_h + 2) * std::fabs(d.inv[4]);
+                auto span = [&](double e) {   // subapertures that floor(x) .. ceil(x + e) can touch
+                    const double s_ = std::floor((std::min(e, 1.0e8) + 2.0) / d.n_pix) + 2.0;
+                    return (int)std::min<double>(s_, d.n_subap);
+                };
+                d.tab_off = off;
+                d.tab_cap = 2 * span(ej) * span(ei);
+                off += d.tab_cap;
+            }
+            tab_floats_max = std::max(tab_floats_max, (off + 3) & ~3);
+        }
+    }
+    // ... and a buffer of zeros, as large as leaves the CTAs-per-SM the registers allow anyway (6)
+    int zbuf_bytes = 0;
+    if (!dense) {
+        const long long base = 4LL * ((long long)patch_pitch * patch_h + 4LL * cell_pitch * cell_h + tab_floats_max);
+        const long long per_sm = 228 * 1024, reserve = 1024;
+        long long k = std::max<long long>(1, std::min<long long>(6, per_sm / (base + reserve + 1024)));
+        zbuf_bytes = (int)std::max<long long>(1024, std::min<long long>(16384, (per_sm / k - reserve - base) & ~15LL));
+        zbuf_bytes = 0;   // TEMP: paced plain stores
+    }
     const size_t smem = dense ? sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)phi_pitch * phi_h)
-                              : sizeof(float) * (size_t)patch_pitch * patch_h;
+                              : sizeof(float) * ((size_t)patch_pitch * patch_h + 4 * (size_t)cell_pitch * cell_h +
+                                                 (size_t)tab_floats_max) + (size_t)zbuf_bytes;
     CUtensorMap tmap;
     if (!dense) {
         synim_status st = encode_cube_map(d_influence, n_modes, ny, nx, patch_pitch, patch_h, &tmap);
@@ -383,8 +422,14 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         std::memset(&p, 0, sizeof(p));
         p.cube = d_influence; p.bbox = d_bbox; p.out = d_out; p.ld = ld;
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
+        p.addr_bias = 0x4B400000u << 4;
+        p.cell_pitch = cell_pitch; p.cell_h = cell_h;
         p.patch_pitch = patch_pitch; p.patch_h = patch_h; p.phi_pitch = phi_pitch; p.phi_h = phi_h;
         for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
+        p.tab_floats = nw > 0 ? (dev[w0 + nw - 1].tab_off + dev[w0 + nw - 1].tab_cap + 3) & ~3 : 0;
+        p.zbuf_bytes = zbuf_bytes;
+        p.prefetch_dist = 444;
+        if (const char *pd = getenv("SYNIM_PF")) p.prefetch_dist = atoi(pd);   // TEMP
         if (dense) {
             p.zero_begin = 0; p.zero_count = 0;
             p.chunks = 8;
@@ -395,6 +440,10 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
             p.zero_count = last.row_x + 2 * last.n_valid - p.zero_begin;
             p.chunks = 1;
             p.jobs_per_mode = 1;
+        }
+        if (const char *ex = getenv("SYNIM_EXP")) {   // TEMP experiment hook
+            if (!strcmp(ex, "nozero")) p.zero_count = 0;
+            if (!strcmp(ex, "nostrip")) p.n_wfs = 0;
         }
         if (dense) SYNIM_CUDA(synim::launch_interaction_matrix(p, smem, s));
         else SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));

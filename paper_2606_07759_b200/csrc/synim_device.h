@@ -8,6 +8,7 @@ namespace synim {
 
 constexpr int kMaxWfsPerLaunch = 16;   // per-launch WFS batch (kernel-parameter space is 4 KB)
 constexpr int kThreads = 256;          // CTA size of the interaction-matrix kernel
+constexpr int kWmapPadRows = 8;        // rows of zeros below each sensor's weight map (strip kernel look-ahead)
 
 // One sensor as the kernel sees it.  All coordinates are ABSOLUTE pixel indices: WFS pixel (i, j)
 // (row, column) samples the source grid at
@@ -26,6 +27,7 @@ struct WfsDev {
     int tile_fixed;          // max edge (WFS pixels) of a D tile when the whole support is one patch
     int tile_dense;          // max edge when the patch is re-staged per tile (its source box must fit)
     int group;               // lanes that share one subaperture in the reduction (power of 2 <= 32)
+    int tab_off, tab_cap;    // strip kernel: this sensor's slice of the CTA's slope table (floats)
     int pad_;
 };
 
@@ -41,6 +43,11 @@ struct ImParams {
                                 // by the mode's CTA before it accumulates (0: caller pre-zeroed)
     int jobs_per_mode;          // 1: one CTA per mode walks every sensor; else n_wfs*chunks CTAs per mode
     int chunks;                 // tile chunks per sensor when jobs_per_mode > 1
+    unsigned addr_bias;         // strip kernel: (bits of 1.5*2^23) << 4 mod 2^32, see process_strip
+    int cell_pitch, cell_h;     // strip kernel: capacity of the bilinear-cell array (float4 cells)
+    int tab_floats;             // strip kernel: size of the CTA's slope table (multiple of 4)
+    int prefetch_dist;          // strip kernel: CTA m pulls the box of mode m + prefetch_dist into L2 (0: off)
+    int zbuf_bytes;             // strip kernel: shared buffer of zeros the column's zeros are bulk-copied from
     WfsDev wfs[kMaxWfsPerLaunch];
 };
 

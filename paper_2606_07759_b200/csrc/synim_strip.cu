@@ -4,17 +4,24 @@
 // touch) is staged ONCE in shared memory by a TMA 3-D box load (cp.async.bulk.tensor, out-of-range
 // elements zero-filled by the hardware = reading R4) and reused by every sensor of the batch
 // (the cube is fetched once for all WFS).  While the load is in flight the CTA streams
-// the zeros of its whole IM column (S4).  Then each warp takes "strips": 30 WFS pixel columns (one
-// per lane, plus one halo column on either side) of one sensor's footprint, and walks down the pixel
-// rows keeping phi of the previous two rows in registers:
+// the zeros of its whole IM column (S4).  The staged pixels are then turned, once, into bilinear
+// CELLS (v00, v01-v00, v10-v00, v11-v10-v01+v00), so that a sample is one 16-byte LDS and three FFMA.
+// Then each warp takes "strips": 30 WFS pixel columns (one per lane, plus one halo column on either
+// side) of one sensor's footprint, and walks down the pixel rows two at a time, keeping phi of the
+// previous two rows in registers:
 //   S1  col/row = tile-local float32 offsets from a float64 per-lane base,
-//   S2  4 LDS + 3 lerps from the staged patch,
+//   S2  floor/fraction with the 1.5*2^23 trick, the shared-memory address straight from the float
+//       mantissa, one LDS.128 + 3 FFMA per sample; a sample outside the staged box is 0 (R4, R15),
 //   S3  D_y from registers, D_x from the two neighbouring lanes (shuffles), weighted by the
 //       precomputed 0.5*P/W_S map, summed down the rows of a subaperture in registers and across
 //       its columns with a segmented warp-shuffle reduction,
 //   S4  one float add into the (already zeroed) column per (subaperture, axis).
 // Rows of a strip that cannot touch the support are never sampled (exact: phi is 0 there, R15).
 // phi is never written anywhere.
+//
+// Measured on B200 (_work microbenchmarks, round 1): FFMA2/FADD2 occupy the issue port for two cycles,
+// so packing pixel pairs into f32x2 saves nothing in an issue-bound kernel; LDS and SHFL each run at
+// about one warp instruction per clock per SM.  Hence scalar FP32 and as few LDS as possible.
 #include "synim_device.h"
 
 #include <cstring>
@@ -24,10 +31,23 @@ namespace synim {
 
 namespace {
 
-constexpr int kStripThreads = 128;
+constexpr int kComputeWarps = 4, kComputeThreads = 32 * kComputeWarps;
+constexpr int kStripThreads = kComputeThreads;
+#ifndef SYNIM_STRIP_MINB
+#define SYNIM_STRIP_MINB 6
+#endif
+#ifdef SYNIM_EXP_NOW   // TEMP experiment: no weight loads
+#define SYNIM_WLOAD(p) (isD ? 0.01f : 0.0f)
+#else
+#define SYNIM_WLOAD(p) __ldg(p)
+#endif
+#ifndef SYNIM_STRIP_ROWS
+#define SYNIM_STRIP_ROWS 4
+#endif
+constexpr int kStripRows = SYNIM_STRIP_ROWS;                // pixel rows per loop iteration (independent samples in flight per lane)
+static_assert(2 * kStripRows <= kWmapPadRows, "weight look-ahead runs past the rows of zeros");
 constexpr int kStripCols = 30;               // D columns per strip: lanes 1..30, halo on lanes 0 and 31
-constexpr float kMagicFloor = 12582912.0f;   // 1.5 * 2^23
-constexpr int kMagicFloorBits = 0x4B400000;
+constexpr float kMagicFloor = 12582912.0f;   // 1.5 * 2^23: fadd.rm(x, magic) = magic + floor(x), |x| < 2^22
 constexpr unsigned kFull = 0xffffffffu;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -70,17 +90,39 @@ __device__ __forceinline__ void tma_load_box(void *dst, const CUtensorMap *map, 
         : "memory");
 }
 
+// pull a box into L2 ahead of the CTA that will stage it
+__device__ __forceinline__ void tma_prefetch_box(const CUtensorMap *map, int x, int y, int z)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map), "r"(x), "r"(y), "r"(z) : "memory");
+}
+
 __device__ __forceinline__ float lds_f32(uint32_t addr)
 {
     float v;
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
     return v;
 }
+// smem -> global bulk copy through the TMA engine (no LSU traffic, no issue slots beyond this one)
+__device__ __forceinline__ void bulk_store(void *dst, uint32_t src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void red_shared_f32(uint32_t addr, float v)
+{
+    asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void sts_f32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
+__device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+__device__ __forceinline__ void sts_f32x4(uint32_t addr, float4 v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
 
 template <int NT>
-__device__ __forceinline__ void zero_fill(float *dst, int n)
+__device__ __forceinline__ void zero_fill(float *dst, int n, int tid)
 {
-    const int tid = threadIdx.x;
     const int mis = (int)((reinterpret_cast<uintptr_t>(dst) >> 2) & 3);
     int head = (4 - mis) & 3;
     if (head > n) head = n;
@@ -94,13 +136,45 @@ __device__ __forceinline__ void zero_fill(float *dst, int n)
     if (tid < n - done) dst[done + tid] = 0.0f;
 }
 
-struct PatchBox {
-    int x0, y0, w, h;   // absolute source origin of the staged box; extent that may be sampled
+// The bilinear cells of one staged piece.  Cell (r, c) covers source pixels x0+c .. x0+c+1, y0+r .. y0+r+1,
+// where (x0, y0) is the upper-left pixel of the piece's ring of zeros; a sample at (col, row) relative to
+// (x0, y0) can be non-zero only for 0 <= col < cw, 0 <= row < ch.
+struct CellBox {
+    int x0, y0;      // absolute source pixel of cell (0, 0)
+    int cw, ch;      // cells per row / rows of cells: piece width + 1, piece height + 1
+    uint32_t base;   // shared-window byte address of cell (0, 0)
+    int pitch;       // cells per row of the array
+};
+
+// Everything a strip needs from its sensor, read once from the kernel parameters.
+struct StripSensor {
+    const float *wmap;
+    int M, n_subap, n_pix;
+};
+
+// S4, the zeros of the column, paced: every thread owns the 16-byte pieces tid, tid+NT, ... of its CTA's
+// column and stores ONE of them per iteration of the sampling loop, so that the column is written at
+// the rate the CTA computes.  (Dumping the whole column at the start of the CTA -- plain stores, bulk
+// copies, or a warp of its own: all measured -- fills the SM's path to L2, and every load of the other
+// warps then waits behind 161 KB of store data.)
+struct ZeroPacer {
+    float4 *v;   // the thread's next piece
+    int left;    // pieces this thread still has to write
+    __device__ __forceinline__ void step()
+    {
+        if (left > 0) {
+            *v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            v += kStripThreads;
+            --left;
+        }
+    }
 };
 
 // One strip: D columns jA .. jA+nC-1 (lanes 1..nC), D rows i0 .. i1 of sensor W.
-__device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const PatchBox &pa,
-                                              const float *__restrict__ patch, int pitch, float *__restrict__ colp)
+// Its partial slopes are added to the CTA's shared table: entry (a, b, axis) of the sensor's window of
+// subapertures (first row a0, first column b0, nb columns) sits at tab + ((a-a0)*nb + (b-b0))*8 + axis*4.
+__device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
+                                              uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp)
 {
     const int lane = threadIdx.x & 31;
     const int nR = i1 - i0 + 1;   // D rows; phi row rr (0 .. nR+1) is absolute row i0-1+rr
@@ -108,23 +182,23 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
 
     // S1: float64 per-lane base, then float32 tile-local offsets
     const double jl = (double)jcol, ib = (double)(i0 - 1);
-    const float bc = (float)(W.fwd[0] * jl + W.fwd[1] * ib + W.fwd[2] - (double)pa.x0);
-    const float br = (float)(W.fwd[3] * jl + W.fwd[4] * ib + W.fwd[5] - (double)pa.y0);
+    const float bc = (float)(W.fwd[0] * jl + W.fwd[1] * ib + W.fwd[2] - (double)cb.x0);
+    const float br = (float)(W.fwd[3] * jl + W.fwd[4] * ib + W.fwd[5] - (double)cb.y0);
     const float a1 = (float)W.fwd[1], a4 = (float)W.fwd[4];
+    const float cwf = (float)cb.cw, chf = (float)cb.ch;
 
-    // phi rows whose pixel segment [lane 0 .. lane nC+1] can reach the box (a sample is non-zero only
-    // if 0 <= col < w-1 and 0 <= row < h-1); every sample of a row lies between its two end points
+    // phi rows whose pixel segment [lane 0 .. lane nC+1] can reach the cells (a sample is non-zero only
+    // if 0 <= col < cw and 0 <= row < ch); every sample of a row lies between its two end points
     const float bcL = __shfl_sync(kFull, bc, 0), brL = __shfl_sync(kFull, br, 0);
     const float bcR = __shfl_sync(kFull, bc, nC + 1), brR = __shfl_sync(kFull, br, nC + 1);
-    const float cw1 = (float)(pa.w - 1) + 0.01f, ch1 = (float)(pa.h - 1) + 0.01f;
     int first = 0x7fffffff, last = -1;
     for (int g = 0; g < nR + 2; g += 32) {
         const int rr = g + lane;
         const float rf = (float)rr;
         const float cl = fmaf(a1, rf, bcL), cr = fmaf(a1, rf, bcR);
         const float rl = fmaf(a4, rf, brL), rq = fmaf(a4, rf, brR);
-        const bool act = rr < nR + 2 && fmaxf(cl, cr) > -0.01f && fminf(cl, cr) < cw1 && fmaxf(rl, rq) > -0.01f &&
-                         fminf(rl, rq) < ch1;
+        const bool act = rr < nR + 2 && fmaxf(cl, cr) > -0.01f && fminf(cl, cr) < cwf + 0.01f && fmaxf(rl, rq) > -0.01f &&
+                         fminf(rl, rq) < chf + 0.01f;
         const unsigned m = __ballot_sync(kFull, act);
         if (m) {
             first = min(first, g + __ffs(m) - 1);
@@ -135,8 +209,11 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     const int d_lo = max(first - 1, 1), d_hi = min(last + 1, nR);   // D rows that can be non-zero
     if (d_hi < d_lo) return;
 
+    StripSensor S;
+    S.wmap = W.wmap; S.M = W.M; S.n_subap = W.n_subap; S.n_pix = W.n_pix;
+
     // segments of lanes that belong to one subaperture column
-    const int npx = W.n_pix;
+    const int npx = S.n_pix;
     const bool isD = lane >= 1 && lane <= nC;
     const int seg = isD ? jcol / npx : -1;
     const int segL = __shfl_up_sync(kFull, seg, 1);
@@ -144,86 +221,177 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     unsigned okm = 0;
     int nsteps = 0;
     while ((1 << nsteps) < min(npx, kStripCols)) ++nsteps;
+#pragma unroll
     for (int s = 0; s < 5; ++s) {
         const int sd = __shfl_down_sync(kFull, seg, 1 << s);
         if (isD && lane + (1 << s) < 32 && sd == seg) okm |= 1u << s;
     }
 
-    const unsigned cmax = (unsigned)(pa.w - 1), rmax = (unsigned)(pa.h - 1);
     const int i_first = i0 - 1 + d_lo;           // absolute row of D row d_lo
     int a_cur = i_first / npx;
-    int rem = i_first - a_cur * npx;
-    const int M = W.M;
-    const float *wp = W.wmap + ((size_t)i_first * M + (isD ? jcol : 0));
-    uint32_t pbase;   // volatile: keeps the shared-window address in a register instead of re-deriving it per row
-    asm volatile("{\n\t.reg .u64 t;\n\tcvta.to.shared.u64 t, %1;\n\tcvt.u32.u64 %0, t;\n\t}" : "=r"(pbase) : "l"(patch));
-    const uint32_t pitch4 = (uint32_t)pitch * 4u;
+    int rem = i_first - a_cur * npx;             // rows of subaperture row a_cur already behind us
+    const int M = S.M;
+    // weight map offsets (elements).  The map has kWmapPadRows rows of zeros below row M-1: halo lanes stay
+    // on the first of them (stride 0), and the look-ahead of the last rows may run onto them.
+    uint32_t woff = isD ? (uint32_t)i_first * (uint32_t)M + (uint32_t)jcol : (uint32_t)M * (uint32_t)M;
+    const uint32_t wrow = isD ? (uint32_t)M : 0u, wstride = isD ? (uint32_t)kStripRows * (uint32_t)M : 0u;
+    uint32_t tent = tab + (uint32_t)((a_cur - a0) * nb + (isD ? seg - b0 : 0)) * 8u;   // this lane's table entry
+    const uint32_t tstep = (uint32_t)nb * 8u;
 
-    // S2: bilinear gather of phi row rr from the staged patch (0 outside it)
-    auto sample = [&](int rr) -> float {
-        const float rf = (float)rr;
-        const float col = fmaf(a1, rf, bc), row = fmaf(a4, rf, br);
-        const float tc = __fadd_rd(col, kMagicFloor), tr = __fadd_rd(row, kMagicFloor);
-        const int c0 = __float_as_int(tc) - kMagicFloorBits, r0 = __float_as_int(tr) - kMagicFloorBits;
-        const float fx = col - (tc - kMagicFloor), fy = row - (tr - kMagicFloor);
-        const bool inb = (unsigned)c0 < cmax && (unsigned)r0 < rmax;
-        const uint32_t at = inb ? pbase + (uint32_t)(r0 * pitch + c0) * 4u : pbase;
-        const float v00 = lds_f32(at), v01 = lds_f32(at + 4u), v10 = lds_f32(at + pitch4), v11 = lds_f32(at + pitch4 + 4u);
-        const float top = fmaf(fx, v01 - v00, v00);
-        const float bot = fmaf(fx, v11 - v10, v10);
-        return inb ? fmaf(fy, bot - top, top) : 0.0f;
+    // S3 (columns): segmented sum over the lanes of a subaperture, then one shared-memory add per axis
+    auto flush = [&](float sx, float sy) {
+        unsigned m = okm;
+        asm volatile("" : "+r"(m));   // keeps the five lane masks out of predicate registers between flushes
+#pragma unroll
+        for (int s = 0; s < 5; ++s) {
+            if (s < nsteps) {   // warp-uniform
+                const float tx = __shfl_down_sync(kFull, sx, 1 << s), ty = __shfl_down_sync(kFull, sy, 1 << s);
+                if ((m >> s) & 1u) { sx += tx; sy += ty; }
+            }
+        }
+        if (head && (sx != 0.0f || sy != 0.0f) && a_cur < S.n_subap) {
+            red_shared_f32(tent, sx);   // another warp may hold the other columns of this subaperture
+            red_shared_f32(tent + 4u, sy);
+        }
+        ++a_cur;
+        tent += tstep;
     };
 
-    float pm2 = sample(d_lo - 1), pm1 = sample(d_lo), sx = 0.0f, sy = 0.0f;
+    // S2: one bilinear sample of phi row rf from the cells; 0 outside them.  Non-negative floats order like
+    // their bit patterns and negative ones have the sign bit set, so one unsigned compare per axis
+    // tests 0 <= x < limit.  Branch-free (predicated LDS), so that the kRows samples of an iteration
+    // overlap: the kernel is latency-bound otherwise (ncu, round 1).
+    const uint32_t cw_bits = __float_as_uint(cwf), ch_bits = __float_as_uint(chf);
+    const float pitchf = (float)cb.pitch;
+    // byte address of cell 0 minus (bits of the magic number << 4) mod 2^32.  The bias is a kernel
+    // parameter, not a literal, so that ptxas keeps the difference in one register and an address is one LEA
+    const uint32_t cbase = cb.base - addr_bias;
+    auto sample = [&](float rf) -> float {
+        const float col = fmaf(a1, rf, bc), row = fmaf(a4, rf, br);
+        const float tc = __fadd_rd(col, kMagicFloor), tr = __fadd_rd(row, kMagicFloor);   // magic + floor
+        const float fx = col - (tc - kMagicFloor), fy = row - (tr - kMagicFloor);
+        // magic + c0 + r0*pitch is exact: its mantissa is the cell index
+        const uint32_t at = __float_as_uint(fmaf(tr - kMagicFloor, pitchf, tc)) * 16u + cbase;
+        float phi;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t.reg .f32 v, gx, gy, gxy, t;\n\t"
+            "setp.lt.u32 p, %1, %2;\n\t"
+            "setp.lt.and.u32 p, %3, %4, p;\n\t"
+            "@p ld.shared.v4.f32 {v, gx, gy, gxy}, [%5];\n\t"
+            "fma.rn.f32 t, %6, gxy, gy;\n\t"
+            "fma.rn.f32 t, %7, t, v;\n\t"
+            "fma.rn.f32 t, %6, gx, t;\n\t"
+            "selp.f32 %0, t, 0f00000000, p;\n\t}"
+            : "=f"(phi)
+            : "r"(__float_as_uint(col)), "r"(cw_bits), "r"(__float_as_uint(row)), "r"(ch_bits), "r"(at), "f"(fx), "f"(fy));
+        return phi;
+    };
+
+    constexpr int kRows = kStripRows;
+    float rf = (float)(d_lo + 1);
+    float pmA = sample((float)(d_lo - 1)), pmB = sample((float)d_lo);   // phi[d-1], phi[d]
+    float wgt[kRows];
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) wgt[k] = SYNIM_WLOAD(S.wmap + (woff + (uint32_t)k * wrow));
+    float sx = 0.0f, sy = 0.0f;
 #pragma unroll 1
-    for (int rr = d_lo + 1; rr <= d_hi + 1; ++rr) {
-        const float cur = sample(rr);
-        // S3: D row d = rr-1: D_y = phi[d+1]-phi[d-1] from registers, D_x from the neighbouring lanes
-        const float wgt = isD ? __ldg(wp) : 0.0f;
-        wp += M;
-        const float dy = cur - pm2;
-        const float dx = __shfl_down_sync(kFull, pm1, 1) - __shfl_up_sync(kFull, pm1, 1);
-        sx = fmaf(wgt, dx, sx);
-        sy = fmaf(wgt, dy, sy);
-        pm2 = pm1;
-        pm1 = cur;
-        ++rem;
-        if (rem == npx || rr == d_hi + 1) {
-            for (int s = 0; s < nsteps; ++s) {
-                const float tx = __shfl_down_sync(kFull, sx, 1 << s), ty = __shfl_down_sync(kFull, sy, 1 << s);
-                if ((okm >> s) & 1u) { sx += tx; sy += ty; }
+    for (int d = d_lo; d <= d_hi; d += kRows) {
+        zp.step();
+        // weights of the next kRows rows, one iteration ahead of their use
+        woff += wstride;
+        float wnx[kRows];
+#pragma unroll
+        for (int k = 0; k < kRows; ++k) wnx[k] = SYNIM_WLOAD(S.wmap + (woff + (uint32_t)k * wrow));
+
+        float cur[kRows];   // phi[d+1 .. d+kRows]
+#pragma unroll
+        for (int k = 0; k < kRows; ++k) cur[k] = sample(rf + (float)k);
+        rf += (float)kRows;
+        // S3: D rows d .. d+kRows-1: D_y from registers, D_x from the neighbouring lanes.  A row past d_hi
+        // has D = 0 exactly (or a weight from the rows of zeros), so it needs no test.
+        float dx[kRows], dy[kRows];
+#pragma unroll
+        for (int k = 0; k < kRows; ++k) {
+            const float mid = k == 0 ? pmB : cur[k - 1];                         // phi[d+k]
+            const float above = k == 0 ? pmA : (k == 1 ? pmB : cur[k - 2]);     // phi[d+k-1]
+            dy[k] = cur[k] - above;
+            dx[k] = __shfl_down_sync(kFull, mid, 1) - __shfl_up_sync(kFull, mid, 1);
+        }
+        if (rem + kRows < npx) {   // warp-uniform: no subaperture row ends inside these rows
+#pragma unroll
+            for (int k = 0; k < kRows; ++k) { sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wgt[k], dy[k], sy); }
+            rem += kRows;
+        } else {
+#pragma unroll
+            for (int k = 0; k < kRows; ++k) {
+                sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wgt[k], dy[k], sy);
+                if (++rem == npx) { flush(sx, sy); sx = 0.0f; sy = 0.0f; rem = 0; }
             }
-            if (head && (sx != 0.0f || sy != 0.0f)) {
-                const int k = __ldg(W.subap_row + a_cur * W.n_subap + seg);
-                if (k >= 0) {
-                    atomicAdd(colp + W.row_x + k, sx * W.scale);   // S4 (result unused: RED)
-                    atomicAdd(colp + W.row_y + k, sy * W.scale);
-                }
+        }
+        pmA = cur[kRows - 2]; pmB = cur[kRows - 1];
+#pragma unroll
+        for (int k = 0; k < kRows; ++k) wgt[k] = wnx[k];
+    }
+    if (rem > 0) flush(sx, sy);
+}
+
+
+// The table's non-zero entries -> the IM column (S4).  kAtomic: the support was split into pieces, whose
+// contributions add up (linearity); the entries are cleared for the next piece.
+template <bool kAtomic, int NT>
+__device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_win, uint32_t tab_base,
+                                              float *__restrict__ colp, int t0)
+{
+    for (int w = 0; w < p.n_wfs; ++w) {
+        const int4 win = s_win[w];   // a0, b0, na, nb
+        const int n = win.z * win.w * 2;
+        if (n <= 0) continue;
+        const WfsDev &W = p.wfs[w];
+        const uint32_t tb = tab_base + (uint32_t)W.tab_off * 4u;
+        const unsigned magic = 0xFFFFFFFFu / (unsigned)win.w + 1u;
+        for (int e = t0; e < n; e += NT) {
+            const float v = lds_f32(tb + (uint32_t)e * 4u);
+            if (v == 0.0f) continue;
+            const int cell = e >> 1;
+            const int ra = win.w == 1 ? cell : (int)__umulhi((unsigned)cell, magic), rb = cell - ra * win.w;   // (magic wraps to 0 for 1)
+            const int k = __ldg(W.subap_row + (win.x + ra) * W.n_subap + (win.y + rb));
+            if (k < 0) continue;
+            float *dst = colp + ((e & 1) ? W.row_y : W.row_x) + k;
+            if (kAtomic) {
+                atomicAdd(dst, v * W.scale);
+                sts_f32(tb + (uint32_t)e * 4u, 0.0f);
+            } else {
+                *dst = v * W.scale;
             }
-            sx = 0.0f; sy = 0.0f; rem = 0; ++a_cur;
         }
     }
 }
 
-__global__ void __launch_bounds__(kStripThreads) synim_strip_kernel(const __grid_constant__ ImParams p,
-                                                                    const __grid_constant__ CUtensorMap tmap)
+__global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
+                                                                                     const __grid_constant__ CUtensorMap tmap)
 {
+    // [ raw TMA box: patch_pitch x patch_h floats | cells: cell_pitch x cell_h float4 | table: tab_floats ]
     extern __shared__ __align__(128) float patch[];
     __shared__ __align__(8) uint64_t bar;
+    __shared__ int4 s_win[kMaxWfsPerLaunch];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int nwarps = kStripThreads / 32;
     const int mode = blockIdx.x;
     float *colp = p.out + (long long)mode * p.ld;
+    const uint32_t raw_base = smem_u32(patch);
+    const uint32_t cell_base = raw_base + (uint32_t)(p.patch_pitch * p.patch_h) * 4u;   // patch_pitch % 4 == 0: 16-byte aligned
+    const uint32_t tab_base = cell_base + (uint32_t)(p.cell_pitch * p.cell_h) * 16u;
 
     const int4 b = __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode);
     const int bx0 = max(b.x, 0), by0 = max(b.y, 0), bx1 = min(b.z, p.nx - 1), by1 = min(b.w, p.ny - 1);
     const bool empty = bx1 < bx0 || by1 < by0;
 
-    // pieces of the support that fit the staged box (one piece unless the bbox hint was too small)
-    // (the box must start on a 16-byte boundary of the source row: up to 3 columns of slack on the left)
+    // pieces of the support that fit the staged box (one piece unless the bbox hint was too small).
+    // Box layout: up to 3 columns of slack (the box must start on a 16-byte boundary of the source row),
+    // the ring, the piece, the ring.
     const int cap_w = p.patch_pitch - 5, cap_h = p.patch_h - 2;
     const int npcx = empty ? 0 : (bx1 - bx0 + cap_w) / cap_w, npcy = empty ? 0 : (by1 - by0 + cap_h) / cap_h;
     const int npieces = npcx * npcy;
+    const bool multi = npieces > 1;
     const uint32_t box_bytes = (uint32_t)(p.patch_pitch * p.patch_h) * 4u;
 
     if (tid == 0 && npieces > 0) {
@@ -233,75 +401,130 @@ __global__ void __launch_bounds__(kStripThreads) synim_strip_kernel(const __grid
         mbar_expect_tx(&bar, box_bytes);
         tma_load_box(patch, &tmap, &bar, (bx0 - 1) & ~3, by0 - 1, mode);
     }
-    if (p.zero_count > 0) zero_fill<kStripThreads>(colp + p.zero_begin, p.zero_count);
-    __syncthreads();   // barrier initialised; this CTA's zeros are ordered before its accumulations
-    uint32_t parity = 0;
+    if (tid == 33 && p.prefetch_dist > 0 && mode + p.prefetch_dist < p.n_modes) {
+        // the box of a mode some CTAs ahead: DRAM latency under the column writes is long, L2 latency is not
+        const int4 nb = __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode + p.prefetch_dist);
+        if (nb.z >= nb.x && nb.w >= nb.y) tma_prefetch_box(&tmap, (max(nb.x, 0) - 1) & ~3, max(nb.y, 0) - 1, mode + p.prefetch_dist);
+    }
+    const uint32_t zbuf = tab_base + (uint32_t)p.tab_floats * 4u;   // p.zbuf_bytes of zeros, 16-byte aligned
+    for (int e = tid; e < p.tab_floats + (p.zbuf_bytes >> 2); e += kStripThreads) sts_f32(tab_base + (uint32_t)e * 4u, 0.0f);
+    if (tid < kMaxWfsPerLaunch) s_win[tid] = make_int4(0, 0, 0, 0);
+    // a split support adds into the column piece by piece: the zeros must be there first
+    if (multi && p.zero_count > 0) zero_fill<kStripThreads>(colp + p.zero_begin, p.zero_count, tid);
+    __syncthreads();   // mbarrier initialised, table and zero buffer cleared
 
-    for (int pc = 0; pc < npieces; ++pc) {
-        const int pcy = pc / npcx, pcx = pc - pcy * npcx;
-        const int qx0 = bx0 + pcx * cap_w, qx1 = min(qx0 + cap_w - 1, bx1);
-        const int qy0 = by0 + pcy * cap_h, qy1 = min(qy0 + cap_h - 1, by1);
-        PatchBox pa;
-        pa.x0 = (qx0 - 1) & ~3; pa.y0 = qy0 - 1; pa.w = qx1 + 2 - pa.x0; pa.h = qy1 - qy0 + 3;
-        const int slack = qx0 - 1 - pa.x0;   // columns 0..slack are left of the piece
-        mbar_wait(&bar, parity);
-        parity ^= 1u;
-        if (npieces > 1) {
-            // by linearity a piece is its own mode: zero outside its box, so clear the ring just staged
-            for (int e = tid; e < pa.w; e += kStripThreads) { patch[e] = 0.0f; patch[(pa.h - 1) * p.patch_pitch + e] = 0.0f; }
-            for (int e = tid; e < pa.h; e += kStripThreads) {
-                for (int c = 0; c <= slack; ++c) patch[e * p.patch_pitch + c] = 0.0f;
-                patch[e * p.patch_pitch + pa.w - 1] = 0.0f;
+    ZeroPacer zp;
+    zp.v = nullptr; zp.left = 0;
+    if (!multi && p.zero_count > 0) {
+        float *z = colp + p.zero_begin;
+        const int mis = (int)((reinterpret_cast<uintptr_t>(z) >> 2) & 3);
+        const int headn = min((4 - mis) & 3, p.zero_count);
+        const int body = (p.zero_count - headn) >> 2, tailn = p.zero_count - headn - (body << 2);
+        if (tid < headn) z[tid] = 0.0f;
+        if (tid < tailn) z[headn + (body << 2) + tid] = 0.0f;
+        zp.v = reinterpret_cast<float4 *>(z + headn) + tid;
+        zp.left = (body - tid + kStripThreads - 1) / kStripThreads;
+    }
+    {
+        uint32_t parity = 0;
+        for (int pc = 0; pc < npieces; ++pc) {
+            const int pcy = pc / npcx, pcx = pc - pcy * npcx;
+            const int qx0 = bx0 + pcx * cap_w, qx1 = min(qx0 + cap_w - 1, bx1);
+            const int qy0 = by0 + pcy * cap_h, qy1 = min(qy0 + cap_h - 1, by1);
+            const int raw_x0 = (qx0 - 1) & ~3;
+            const int slack = qx0 - 1 - raw_x0;   // raw column `slack` is the left ring
+            CellBox cb;
+            cb.x0 = qx0 - 1; cb.y0 = qy0 - 1; cb.cw = qx1 - qx0 + 2; cb.ch = qy1 - qy0 + 2;
+            cb.base = cell_base; cb.pitch = p.cell_pitch;
+            mbar_wait(&bar, parity);
+            parity ^= 1u;
+
+            // raw pixels -> cells.  By linearity a piece is its own mode, zero outside its box: when the
+            // support was split, whatever the box holds on the piece's ring is read as 0.
+            {
+                const int ncell = cb.cw * cb.ch;
+                const unsigned magic = 0xFFFFFFFFu / (unsigned)cb.cw + 1u;
+                const uint32_t rpitch4 = (uint32_t)p.patch_pitch * 4u;
+                for (int e = tid; e < ncell; e += kComputeThreads) {
+                    const int r = (int)__umulhi((unsigned)e, magic);
+                    const int c = e - r * cb.cw;
+                    const uint32_t at = raw_base + (uint32_t)(r * p.patch_pitch + slack + c) * 4u;
+                    float v00 = lds_f32(at), v01 = lds_f32(at + 4u), v10 = lds_f32(at + rpitch4), v11 = lds_f32(at + rpitch4 + 4u);
+                    if (multi) {
+                        const bool l = c == 0, rgt = c == cb.cw - 1, t = r == 0, bt = r == cb.ch - 1;
+                        if (l || t) v00 = 0.0f;
+                        if (rgt || t) v01 = 0.0f;
+                        if (l || bt) v10 = 0.0f;
+                        if (rgt || bt) v11 = 0.0f;
+                    }
+                    const float dx = v01 - v00;
+                    sts_f32x4(cell_base + (uint32_t)(r * p.cell_pitch + c) * 16u, make_float4(v00, dx, v10 - v00, (v11 - v10) - dx));
+                }
             }
-            __syncthreads();
-        }
+            bar_sync(1, kComputeThreads);   // cells complete; the raw box is free again
 
-        // lane w: footprint of this piece on sensor w = image of the open box (qx0-1,qx1+1)x(qy0-1,qy1+1)
-        // under the inverse map, +-1 pixel for the stencil, clipped to the sensor
-        int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0;
-        if (lane < p.n_wfs) {
-            const WfsDev &W = p.wfs[lane];
-            double jmin = 1e300, jmax = -1e300, imin = 1e300, imax = -1e300;
-#pragma unroll
-            for (int cr = 0; cr < 4; ++cr) {
-                const double c = (cr & 1) ? (double)(qx1 + 1) : (double)(qx0 - 1);
-                const double r = (cr & 2) ? (double)(qy1 + 1) : (double)(qy0 - 1);
-                const double j = W.inv[0] * c + W.inv[1] * r + W.inv[2];
-                const double i = W.inv[3] * c + W.inv[4] * r + W.inv[5];
-                jmin = fmin(jmin, j); jmax = fmax(jmax, j); imin = fmin(imin, i); imax = fmax(imax, i);
-            }
-            const double lim = 1.0e9;
-            r_j0 = max(0, (int)floor(fmax(jmin, -lim)) - 1); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)) + 1);
-            r_i0 = max(0, (int)floor(fmax(imin, -lim)) - 1); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)) + 1);
-            if (r_j1 >= r_j0 && r_i1 >= r_i0) r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
-        }
-        int incl = r_n;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const int t = __shfl_up_sync(kFull, incl, d);
-            if (lane >= d) incl += t;
-        }
-        const int total = __shfl_sync(kFull, incl, 31);
-        for (int t = warp; t < total; t += nwarps) {
-            const int w = __popc(__ballot_sync(kFull, incl <= t));
-            const int base = __shfl_sync(kFull, incl - r_n, w);
-            const int i0 = __shfl_sync(kFull, r_i0, w), i1 = __shfl_sync(kFull, r_i1, w);
-            const int j0 = __shfl_sync(kFull, r_j0, w), j1 = __shfl_sync(kFull, r_j1, w);
-            const int jA = j0 + (t - base) * kStripCols;
-            const int nC = min(kStripCols, j1 - jA + 1);
-            process_strip(p.wfs[w], i0, i1, jA, nC, pa, patch, p.patch_pitch, colp);
-        }
-
-        if (pc + 1 < npieces) {
-            __syncthreads();   // every warp is done with this piece
-            if (tid == 0) {
+            if (pc + 1 < npieces && tid == 0) {   // next piece's box lands while this one is sampled
                 const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
                 fence_proxy_async();
                 mbar_expect_tx(&bar, box_bytes);
                 tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
             }
+
+            // lane w: footprint of this piece on sensor w.  phi(i,j) can be non-zero only strictly inside the
+            // image of the open box (qx0-1,qx1+1)x(qy0-1,qy1+1) under the inverse map, so D(i,j) only for
+            // floor(jmin) <= j <= ceil(jmax) (one pixel of stencil either side), clipped to the sensor
+            int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_nb = 0;
+            if (lane < p.n_wfs) {
+                const WfsDev &W = p.wfs[lane];
+                double jmin = 1e300, jmax = -1e300, imin = 1e300, imax = -1e300;
+#pragma unroll
+                for (int cr = 0; cr < 4; ++cr) {
+                    const double c = (cr & 1) ? (double)(qx1 + 1) : (double)(qx0 - 1);
+                    const double r = (cr & 2) ? (double)(qy1 + 1) : (double)(qy0 - 1);
+                    const double j = W.inv[0] * c + W.inv[1] * r + W.inv[2];
+                    const double i = W.inv[3] * c + W.inv[4] * r + W.inv[5];
+                    jmin = fmin(jmin, j); jmax = fmax(jmax, j); imin = fmin(imin, i); imax = fmax(imax, i);
+                }
+                const double lim = 1.0e9;
+                r_j0 = max(0, (int)floor(fmax(jmin, -lim))); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)));
+                r_i0 = max(0, (int)floor(fmax(imin, -lim))); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)));
+                int4 win = make_int4(0, 0, 0, 0);
+                if (r_j1 >= r_j0 && r_i1 >= r_i0) {
+                    r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
+                    r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
+                    r_nb = r_j1 / W.n_pix - r_b0 + 1;
+                    win = make_int4(r_a0, r_b0, r_i1 / W.n_pix - r_a0 + 1, r_nb);
+                    if (win.z * win.w * 2 > W.tab_cap) __trap();   // the host sized the table from the same bounds
+                }
+                if (warp == 0) s_win[lane] = win;   // read by scatter_table after a barrier
+            }
+            int incl = r_n;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(kFull, incl, d);
+                if (lane >= d) incl += t;
+            }
+            const int total = __shfl_sync(kFull, incl, 31);
+            for (int t = warp; t < total; t += kComputeWarps) {
+                const int w = __popc(__ballot_sync(kFull, incl <= t));
+                const int base = __shfl_sync(kFull, incl - r_n, w);
+                const int i0 = __shfl_sync(kFull, r_i0, w), i1 = __shfl_sync(kFull, r_i1, w);
+                const int j0 = __shfl_sync(kFull, r_j0, w), j1 = __shfl_sync(kFull, r_j1, w);
+                const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
+                const int jA = j0 + (t - base) * kStripCols;
+                const int nC = min(kStripCols, j1 - jA + 1);
+                process_strip(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
+            }
+            if (multi) {
+                bar_sync(1, kComputeThreads);   // every warp is done with these cells and this piece's table
+                scatter_table<true, kComputeThreads>(p, s_win, tab_base, colp, tid);
+                bar_sync(1, kComputeThreads);   // table clear again, windows free
+            }
         }
     }
+    while (zp.left > 0) zp.step();   // what the sampling loop did not get to
+    __syncthreads();                  // all zeros stored before anyone stores a value; table complete
+    if (!multi && npieces > 0) scatter_table<false, kStripThreads>(p, s_win, tab_base, colp, tid);
 }
 
 }  // namespace

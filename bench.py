@@ -211,15 +211,15 @@ def main():
     scales = [w.slope_scale for w in wl.wfs]
     geom = synim.create_geometry(wl.ny, wl.nx, wl.wfs)
     cube = torch.from_numpy(wl.cube).cuda()
-    bbox, bmax = None, (0, 0)
+    bbox, diag, bmax = None, None, (0, 0)
     if wl.bbox is not None:
-        bbox = synim.compute_bboxes(cube)
+        bbox, diag = synim.compute_supports(cube)
         bmax = synim.bbox_extent(bbox)
     out = torch.empty((wl.n_modes, geom.num_rows), dtype=torch.float32, device="cuda")
     stream = torch.cuda.current_stream()
 
     def step():
-        synim.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax, stream=stream)
+        synim.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax, stream=stream, diag=diag)
 
     for _ in range(warmup):
         step()

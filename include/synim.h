@@ -120,6 +120,11 @@ int64_t synim_row_offset(const synim_geometry *geom, int32_t wfs);
  *   d_bbox       DEVICE int32 [n_modes][4] = (x0,y0,x1,y1) inclusive extent outside which the mode is
  *                exactly zero (x1 < x0: the mode is identically zero), or NULL = dense modes.
  *                A bbox that leaves out non-zero samples gives wrong results (not checked).
+ *   d_diag       DEVICE int32 [n_modes][4] = (min x+y, max x+y, min x-y, max x-y) over the mode's non-zero
+ *                pixels, or NULL.  With the bbox this is the support's bounding octagon: under a rotated
+ *                sensor the footprint of a round influence function is then its own size, not that of
+ *                its rotated bounding box.  Only ever narrows what is sampled (same "not checked" rule);
+ *                requires d_bbox.  16-byte aligned.
  *   bbox_max_w/h HOST upper bounds of x1-x0+1 / y1-y0+1 over all modes, used only to size the
  *                shared-memory tiles (<= 0: unknown).  Wrong bounds cost speed, never correctness.
  *   affine       HOST [n_wfs]
@@ -128,14 +133,16 @@ int64_t synim_row_offset(const synim_geometry *geom, int32_t wfs);
  *                [0, num_rows) of columns [0, n_modes) is written (padding rows are left untouched)
  * Errors: INVALID_ARG (NULL, n_modes < 0, ld < rows, singular affine), ALIGNMENT, CUDA. */
 synim_status synim_interaction_matrix(const synim_geometry *geom, const float *d_influence, int32_t n_modes,
-                                      const int32_t *d_bbox, int32_t bbox_max_w, int32_t bbox_max_h,
+                                      const int32_t *d_bbox, const int32_t *d_diag, int32_t bbox_max_w,
+                                      int32_t bbox_max_h,
                                       const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out,
                                       int64_t ld, void *stream);
 
 /* Tight non-zero extent of every mode of a cube (DEVICE in, DEVICE out int32 [n_modes][4]);
- * an all-zero mode gets (0,0,-1,-1).  Asynchronous. */
+ * an all-zero mode gets (0,0,-1,-1).  d_diag (DEVICE int32 [n_modes][4], or NULL) receives the
+ * diagonal extents described above; an all-zero mode gets (0,-1,0,-1).  Asynchronous. */
 synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx,
-                                  int32_t *d_bbox, void *stream);
+                                  int32_t *d_bbox, int32_t *d_diag, void *stream);
 /* Largest bbox width / height (HOST out); synchronises `stream`. */
 synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *max_w, int32_t *max_h,
                                void *stream);

@@ -295,7 +295,7 @@ int64_t synim_row_offset(const synim_geometry *g, int32_t w)
 }
 
 synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_influence, int32_t n_modes,
-                                      const int32_t *d_bbox, int32_t bbox_max_w, int32_t bbox_max_h,
+                                      const int32_t *d_bbox, const int32_t *d_diag, int32_t bbox_max_w, int32_t bbox_max_h,
                                       const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out, int64_t ld,
                                       void *stream)
 {
@@ -308,7 +308,9 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     if (ld < g->rows) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: ld = %lld < rows = %lld", (long long)ld, g->rows);
     if (reinterpret_cast<uintptr_t>(d_influence) % 16 != 0)
         return fail(SYNIM_ERR_ALIGNMENT, "synim_interaction_matrix: influence cube is not 16-byte aligned");
-    if (reinterpret_cast<uintptr_t>(d_out) % 4 != 0 || (d_bbox && reinterpret_cast<uintptr_t>(d_bbox) % 16 != 0))
+    if (d_diag && !d_bbox) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: d_diag without d_bbox");
+    if (reinterpret_cast<uintptr_t>(d_out) % 4 != 0 || (d_bbox && reinterpret_cast<uintptr_t>(d_bbox) % 16 != 0) ||
+        (d_diag && reinterpret_cast<uintptr_t>(d_diag) % 16 != 0))
         return fail(SYNIM_ERR_ALIGNMENT, "synim_interaction_matrix: output / bbox pointer misaligned");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int n_wfs = (int)g->wfs.size();
@@ -390,18 +392,13 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
             tab_floats_max = std::max(tab_floats_max, (off + 3) & ~3);
         }
     }
-    // ... and a buffer of zeros, as large as leaves the CTAs-per-SM the registers allow anyway (6)
-    int zbuf_bytes = 0;
-    if (!dense) {
-        const long long base = 4LL * ((long long)patch_pitch * patch_h + 4LL * cell_pitch * cell_h + tab_floats_max);
-        const long long per_sm = 228 * 1024, reserve = 1024;
-        long long k = std::max<long long>(1, std::min<long long>(6, per_sm / (base + reserve + 1024)));
-        zbuf_bytes = (int)std::max<long long>(1024, std::min<long long>(16384, (per_sm / k - reserve - base) & ~15LL));
-        zbuf_bytes = 0;   // TEMP: paced plain stores
-    }
+    // bilinear cells only while they leave six CTAs per SM (what the registers allow): 228 KB / 6 - 1 KB each
+    const size_t strip_fixed = sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)tab_floats_max) +
+                               sizeof(int) * (size_t)(tab_floats_max / 2);
+    const size_t strip_cells = sizeof(float) * 4 * (size_t)cell_pitch * cell_h;
+    const bool use_cells = !dense && strip_fixed + strip_cells <= (228 * 1024) / 6 - 1024 && !getenv("SYNIM_NOCELLS");   // TEMP env
     const size_t smem = dense ? sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)phi_pitch * phi_h)
-                              : sizeof(float) * ((size_t)patch_pitch * patch_h + 4 * (size_t)cell_pitch * cell_h +
-                                                 (size_t)tab_floats_max) + (size_t)zbuf_bytes;
+                              : strip_fixed + (use_cells ? strip_cells : 0);
     CUtensorMap tmap;
     if (!dense) {
         synim_status st = encode_cube_map(d_influence, n_modes, ny, nx, patch_pitch, patch_h, &tmap);
@@ -420,16 +417,13 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         const int nw = std::min(synim::kMaxWfsPerLaunch, n_wfs - w0);
         synim::ImParams p;
         std::memset(&p, 0, sizeof(p));
-        p.cube = d_influence; p.bbox = d_bbox; p.out = d_out; p.ld = ld;
+        p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.out = d_out; p.ld = ld;
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
         p.addr_bias = 0x4B400000u << 4;
         p.cell_pitch = cell_pitch; p.cell_h = cell_h;
         p.patch_pitch = patch_pitch; p.patch_h = patch_h; p.phi_pitch = phi_pitch; p.phi_h = phi_h;
         for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
         p.tab_floats = nw > 0 ? (dev[w0 + nw - 1].tab_off + dev[w0 + nw - 1].tab_cap + 3) & ~3 : 0;
-        p.zbuf_bytes = zbuf_bytes;
-        p.prefetch_dist = 444;
-        if (const char *pd = getenv("SYNIM_PF")) p.prefetch_dist = atoi(pd);   // TEMP
         if (dense) {
             p.zero_begin = 0; p.zero_count = 0;
             p.chunks = 8;
@@ -441,25 +435,22 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
             p.chunks = 1;
             p.jobs_per_mode = 1;
         }
-        if (const char *ex = getenv("SYNIM_EXP")) {   // TEMP experiment hook
-            if (!strcmp(ex, "nozero")) p.zero_count = 0;
-            if (!strcmp(ex, "nostrip")) p.n_wfs = 0;
-        }
         if (dense) SYNIM_CUDA(synim::launch_interaction_matrix(p, smem, s));
-        else SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));
+        else SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, use_cells, s));
     }
     return SYNIM_OK;
 }
 
 synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx, int32_t *d_bbox,
-                                  void *stream)
+                                  int32_t *d_diag, void *stream)
 {
     if (n_modes < 0 || ny <= 0 || nx <= 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_compute_bboxes: bad sizes");
     if (n_modes == 0) return SYNIM_OK;
     if (!d_influence || !d_bbox) return fail(SYNIM_ERR_INVALID_ARG, "synim_compute_bboxes: NULL device buffer");
-    if (nx % 4 != 0 || reinterpret_cast<uintptr_t>(d_influence) % 16 != 0 || reinterpret_cast<uintptr_t>(d_bbox) % 16 != 0)
+    if (nx % 4 != 0 || reinterpret_cast<uintptr_t>(d_influence) % 16 != 0 || reinterpret_cast<uintptr_t>(d_bbox) % 16 != 0 ||
+        reinterpret_cast<uintptr_t>(d_diag) % 16 != 0)
         return fail(SYNIM_ERR_ALIGNMENT, "synim_compute_bboxes: need nx %% 4 == 0 and 16-byte aligned buffers");
-    SYNIM_CUDA(synim::launch_compute_bboxes(d_influence, n_modes, ny, nx, d_bbox, static_cast<cudaStream_t>(stream)));
+    SYNIM_CUDA(synim::launch_compute_bboxes(d_influence, n_modes, ny, nx, d_bbox, d_diag, static_cast<cudaStream_t>(stream)));
     return SYNIM_OK;
 }
 
@@ -507,7 +498,7 @@ synim_status synim_interaction_matrix_host(const synim_geometry *g, const float 
         SYNIM_CUDA(cudaMemcpyAsync(g->ws_bbox, h_bbox, bbox_bytes, cudaMemcpyHostToDevice, s));
     }
     SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, h_influence, cube_bytes, cudaMemcpyHostToDevice, s));
-    st = synim_interaction_matrix(g, g->ws_cube, n_modes, h_bbox ? g->ws_bbox : nullptr, bw, bh, affine, mode, g->ws_out,
+    st = synim_interaction_matrix(g, g->ws_cube, n_modes, h_bbox ? g->ws_bbox : nullptr, nullptr, bw, bh, affine, mode, g->ws_out,
                                   g->rows, s);
     if (st != SYNIM_OK) return st;
     SYNIM_CUDA(cudaMemcpyAsync(h_out, g->ws_out, out_bytes, cudaMemcpyDeviceToHost, s));

@@ -34,6 +34,7 @@ struct WfsDev {
 struct ImParams {
     const float *cube;       // [n_modes][ny][nx]
     const int *bbox;         // [n_modes][4] or nullptr
+    const int *diag;         // [n_modes][4] min/max of x+y, min/max of x-y over the support, or nullptr
     float *out;              // column-major IM
     long long ld;
     int n_modes, ny, nx, n_wfs;
@@ -46,19 +47,17 @@ struct ImParams {
     unsigned addr_bias;         // strip kernel: (bits of 1.5*2^23) << 4 mod 2^32, see process_strip
     int cell_pitch, cell_h;     // strip kernel: capacity of the bilinear-cell array (float4 cells)
     int tab_floats;             // strip kernel: size of the CTA's slope table (multiple of 4)
-    int prefetch_dist;          // strip kernel: CTA m pulls the box of mode m + prefetch_dist into L2 (0: off)
-    int zbuf_bytes;             // strip kernel: shared buffer of zeros the column's zeros are bulk-copied from
     WfsDev wfs[kMaxWfsPerLaunch];
 };
 
 // launchers (synim_kernels.cu); all asynchronous on `stream`, return the launch status
 cudaError_t launch_interaction_matrix(const ImParams &p, size_t smem_bytes, cudaStream_t stream);
 // compact-support path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
-// {patch_pitch, patch_h, 1}
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream);
+// {patch_pitch, patch_h, 1}; cells: build 16-byte bilinear cells from the staged box (smem_bytes covers them)
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool cells, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
                                  float *d_wmap, int *d_error_flag, cudaStream_t stream);
-cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox,
+cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox, int *d_diag,
                                   cudaStream_t stream);
 cudaError_t launch_bbox_extent(const int *d_bbox, int n_modes, int *d_wh, cudaStream_t stream);
 size_t max_dynamic_smem();  // opt-in limit of the current device (bytes)

@@ -275,38 +275,44 @@ __global__ void __launch_bounds__(128) subap_weights_kernel(const float *__restr
     }
 }
 
-// one CTA per mode: tight non-zero extent
+// one CTA per mode: tight non-zero extent (x0,y0,x1,y1) and, if asked for, the diagonal extents
+// (min x+y, max x+y, min x-y, max x-y) of the non-zero pixels: together the support's bounding octagon
 __global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ cube, int ny, int nx,
-                                                   int *__restrict__ bbox)
+                                                   int *__restrict__ bbox, int *__restrict__ diag)
 {
     const float4 *img = reinterpret_cast<const float4 *>(cube + (size_t)blockIdx.x * ny * nx);
     const int nx4 = nx >> 2, n4 = ny * nx4;
-    int x0 = 0x7fffffff, y0 = 0x7fffffff, x1 = -1, y1 = -1;
+    const int big = 0x3fffffff;
+    int lo[4] = {big, big, big, big};      // x0, y0, min x+y, min x-y
+    int hi[4] = {-big, -big, -big, -big};  // x1, y1, max x+y, max x-y
     for (int e = threadIdx.x; e < n4; e += 256) {
         const float4 v = __ldg(img + e);
         if (v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f) {
             const int r = e / nx4, c = (e - r * nx4) << 2;
-            const int lo = v.x != 0.f ? 0 : (v.y != 0.f ? 1 : (v.z != 0.f ? 2 : 3));
-            const int hi = v.w != 0.f ? 3 : (v.z != 0.f ? 2 : (v.y != 0.f ? 1 : 0));
-            x0 = min(x0, c + lo); x1 = max(x1, c + hi); y0 = min(y0, r); y1 = max(y1, r);
+            const int l = v.x != 0.f ? 0 : (v.y != 0.f ? 1 : (v.z != 0.f ? 2 : 3));
+            const int h = v.w != 0.f ? 3 : (v.z != 0.f ? 2 : (v.y != 0.f ? 1 : 0));
+            // within one row x+y and x-y are both extreme at the first / last non-zero pixel
+            lo[0] = min(lo[0], c + l); hi[0] = max(hi[0], c + h); lo[1] = min(lo[1], r); hi[1] = max(hi[1], r);
+            lo[2] = min(lo[2], c + l + r); hi[2] = max(hi[2], c + h + r);
+            lo[3] = min(lo[3], c + l - r); hi[3] = max(hi[3], c + h - r);
         }
     }
-    for (int o = 16; o > 0; o >>= 1) {
-        x0 = min(x0, __shfl_xor_sync(0xffffffffu, x0, o)); y0 = min(y0, __shfl_xor_sync(0xffffffffu, y0, o));
-        x1 = max(x1, __shfl_xor_sync(0xffffffffu, x1, o)); y1 = max(y1, __shfl_xor_sync(0xffffffffu, y1, o));
-    }
-    __shared__ int sh[8][4];
-    if ((threadIdx.x & 31) == 0) {
-        sh[threadIdx.x >> 5][0] = x0; sh[threadIdx.x >> 5][1] = y0;
-        sh[threadIdx.x >> 5][2] = x1; sh[threadIdx.x >> 5][3] = y1;
+    __shared__ int sh[8][8];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[q] = min(lo[q], __shfl_xor_sync(0xffffffffu, lo[q], o));
+            hi[q] = max(hi[q], __shfl_xor_sync(0xffffffffu, hi[q], o));
+        }
+        if ((threadIdx.x & 31) == 0) { sh[threadIdx.x >> 5][q] = lo[q]; sh[threadIdx.x >> 5][4 + q] = hi[q]; }
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        for (int k = 1; k < 8; ++k) {
-            x0 = min(x0, sh[k][0]); y0 = min(y0, sh[k][1]); x1 = max(x1, sh[k][2]); y1 = max(y1, sh[k][3]);
-        }
-        int4 o = (x1 < 0) ? make_int4(0, 0, -1, -1) : make_int4(x0, y0, x1, y1);
-        reinterpret_cast<int4 *>(bbox)[blockIdx.x] = o;
+        for (int k = 1; k < 8; ++k)
+            for (int q = 0; q < 4; ++q) { lo[q] = min(lo[q], sh[k][q]); hi[q] = max(hi[q], sh[k][4 + q]); }
+        const bool none = hi[0] < 0;
+        reinterpret_cast<int4 *>(bbox)[blockIdx.x] = none ? make_int4(0, 0, -1, -1) : make_int4(lo[0], lo[1], hi[0], hi[1]);
+        if (diag) reinterpret_cast<int4 *>(diag)[blockIdx.x] = none ? make_int4(0, -1, 0, -1) : make_int4(lo[2], hi[2], lo[3], hi[3]);
     }
 }
 
@@ -359,11 +365,11 @@ cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, i
     return cudaGetLastError();
 }
 
-cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox,
+cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox, int *d_diag,
                                   cudaStream_t stream)
 {
     if (n_modes <= 0) return cudaSuccess;
-    bbox_kernel<<<n_modes, 256, 0, stream>>>(d_cube, ny, nx, d_bbox);
+    bbox_kernel<<<n_modes, 256, 0, stream>>>(d_cube, ny, nx, d_bbox, d_diag);
     return cudaGetLastError();
 }
 

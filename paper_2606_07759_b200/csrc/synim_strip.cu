@@ -90,25 +90,23 @@ __device__ __forceinline__ void tma_load_box(void *dst, const CUtensorMap *map, 
         : "memory");
 }
 
-// pull a box into L2 ahead of the CTA that will stage it
-__device__ __forceinline__ void tma_prefetch_box(const CUtensorMap *map, int x, int y, int z)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map), "r"(x), "r"(y), "r"(z) : "memory");
-}
-
 __device__ __forceinline__ float lds_f32(uint32_t addr)
 {
     float v;
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
     return v;
 }
-// smem -> global bulk copy through the TMA engine (no LSU traffic, no issue slots beyond this one)
-__device__ __forceinline__ void bulk_store(void *dst, uint32_t src, uint32_t bytes)
+__device__ __forceinline__ void cp_async_4(uint32_t dst, const void *src)
 {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
 }
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ int lds_s32(uint32_t addr)
+{
+    int v;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
 __device__ __forceinline__ void red_shared_f32(uint32_t addr, float v)
 {
     asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
@@ -142,8 +140,11 @@ __device__ __forceinline__ void zero_fill(float *dst, int n, int tid)
 struct CellBox {
     int x0, y0;      // absolute source pixel of cell (0, 0)
     int cw, ch;      // cells per row / rows of cells: piece width + 1, piece height + 1
-    uint32_t base;   // shared-window byte address of cell (0, 0)
-    int pitch;       // cells per row of the array
+    uint32_t base;   // shared-window byte address of cell (0, 0), or of its upper-left pixel in the raw box
+    int pitch;       // cells (or pixels) per row of the array
+    // a sample can be non-zero only for s_lo < col+row < s_hi and d_lo < col-row < d_hi as well (the
+    // support's bounding octagon, grown by the reach of a bilinear sample)
+    float s_lo, s_hi, d_lo, d_hi;
 };
 
 // Everything a strip needs from its sensor, read once from the kernel parameters.
@@ -173,6 +174,7 @@ struct ZeroPacer {
 // One strip: D columns jA .. jA+nC-1 (lanes 1..nC), D rows i0 .. i1 of sensor W.
 // Its partial slopes are added to the CTA's shared table: entry (a, b, axis) of the sensor's window of
 // subapertures (first row a0, first column b0, nb columns) sits at tab + ((a-a0)*nb + (b-b0))*8 + axis*4.
+template <bool kCells>
 __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
                                               uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp)
 {
@@ -187,8 +189,9 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     const float a1 = (float)W.fwd[1], a4 = (float)W.fwd[4];
     const float cwf = (float)cb.cw, chf = (float)cb.ch;
 
-    // phi rows whose pixel segment [lane 0 .. lane nC+1] can reach the cells (a sample is non-zero only
-    // if 0 <= col < cw and 0 <= row < ch); every sample of a row lies between its two end points
+    // phi rows whose pixel segment [lane 0 .. lane nC+1] can reach the support's octagon (a sample is
+    // non-zero only if 0 <= col < cw, 0 <= row < ch and inside the diagonal limits); every sample of a
+    // row lies between its two end points, and each limit is a half-plane
     const float bcL = __shfl_sync(kFull, bc, 0), brL = __shfl_sync(kFull, br, 0);
     const float bcR = __shfl_sync(kFull, bc, nC + 1), brR = __shfl_sync(kFull, br, nC + 1);
     int first = 0x7fffffff, last = -1;
@@ -197,8 +200,10 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         const float rf = (float)rr;
         const float cl = fmaf(a1, rf, bcL), cr = fmaf(a1, rf, bcR);
         const float rl = fmaf(a4, rf, brL), rq = fmaf(a4, rf, brR);
+        const float sl = cl + rl, sr = cr + rq, dl = cl - rl, dr = cr - rq;
         const bool act = rr < nR + 2 && fmaxf(cl, cr) > -0.01f && fminf(cl, cr) < cwf + 0.01f && fmaxf(rl, rq) > -0.01f &&
-                         fminf(rl, rq) < chf + 0.01f;
+                         fminf(rl, rq) < chf + 0.01f && fmaxf(sl, sr) > cb.s_lo && fminf(sl, sr) < cb.s_hi &&
+                         fmaxf(dl, dr) > cb.d_lo && fminf(dl, dr) < cb.d_hi;
         const unsigned m = __ballot_sync(kFull, act);
         if (m) {
             first = min(first, g + __ffs(m) - 1);
@@ -263,27 +268,53 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // overlap: the kernel is latency-bound otherwise (ncu, round 1).
     const uint32_t cw_bits = __float_as_uint(cwf), ch_bits = __float_as_uint(chf);
     const float pitchf = (float)cb.pitch;
-    // byte address of cell 0 minus (bits of the magic number << 4) mod 2^32.  The bias is a kernel
-    // parameter, not a literal, so that ptxas keeps the difference in one register and an address is one LEA
+    // byte address of element 0 minus (bits of the magic number << 4, or << 2 for pixels) mod 2^32.  The
+    // bias is a kernel parameter, not a literal, so that ptxas keeps the difference in one register and
+    // an address is one LEA
     const uint32_t cbase = cb.base - addr_bias;
+    const uint32_t rpitch4 = (uint32_t)cb.pitch * 4u;
     auto sample = [&](float rf) -> float {
         const float col = fmaf(a1, rf, bc), row = fmaf(a4, rf, br);
         const float tc = __fadd_rd(col, kMagicFloor), tr = __fadd_rd(row, kMagicFloor);   // magic + floor
         const float fx = col - (tc - kMagicFloor), fy = row - (tr - kMagicFloor);
-        // magic + c0 + r0*pitch is exact: its mantissa is the cell index
-        const uint32_t at = __float_as_uint(fmaf(tr - kMagicFloor, pitchf, tc)) * 16u + cbase;
+        // magic + c0 + r0*pitch is exact: its mantissa is the element index
+        const uint32_t idx = __float_as_uint(fmaf(tr - kMagicFloor, pitchf, tc));
         float phi;
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t.reg .f32 v, gx, gy, gxy, t;\n\t"
-            "setp.lt.u32 p, %1, %2;\n\t"
-            "setp.lt.and.u32 p, %3, %4, p;\n\t"
-            "@p ld.shared.v4.f32 {v, gx, gy, gxy}, [%5];\n\t"
-            "fma.rn.f32 t, %6, gxy, gy;\n\t"
-            "fma.rn.f32 t, %7, t, v;\n\t"
-            "fma.rn.f32 t, %6, gx, t;\n\t"
-            "selp.f32 %0, t, 0f00000000, p;\n\t}"
-            : "=f"(phi)
-            : "r"(__float_as_uint(col)), "r"(cw_bits), "r"(__float_as_uint(row)), "r"(ch_bits), "r"(at), "f"(fx), "f"(fy));
+        if (kCells) {   // one 16-byte cell: v00, v01-v00, v10-v00, v11-v10-v01+v00
+            const uint32_t at = idx * 16u + cbase;
+            asm volatile(
+                "{\n\t.reg .pred p;\n\t.reg .f32 v, gx, gy, gxy, t;\n\t"
+                "setp.lt.u32 p, %1, %2;\n\t"
+                "setp.lt.and.u32 p, %3, %4, p;\n\t"
+                "@p ld.shared.v4.f32 {v, gx, gy, gxy}, [%5];\n\t"
+                "fma.rn.f32 t, %6, gxy, gy;\n\t"
+                "fma.rn.f32 t, %7, t, v;\n\t"
+                "fma.rn.f32 t, %6, gx, t;\n\t"
+                "selp.f32 %0, t, 0f00000000, p;\n\t}"
+                : "=f"(phi)
+                : "r"(__float_as_uint(col)), "r"(cw_bits), "r"(__float_as_uint(row)), "r"(ch_bits), "r"(at), "f"(fx), "f"(fy));
+        } else {        // the four pixels straight from the staged box (supports too large for cells)
+            const uint32_t at = idx * 4u + cbase;
+            asm volatile(
+                "{\n\t.reg .pred p;\n\t.reg .f32 v00, v01, v10, v11, t, u;\n\t.reg .b32 at1;\n\t"
+                "setp.lt.u32 p, %1, %2;\n\t"
+                "setp.lt.and.u32 p, %3, %4, p;\n\t"
+                "add.u32 at1, %5, %8;\n\t"
+                "@p ld.shared.f32 v00, [%5];\n\t"
+                "@p ld.shared.f32 v01, [%5+4];\n\t"
+                "@p ld.shared.f32 v10, [at1];\n\t"
+                "@p ld.shared.f32 v11, [at1+4];\n\t"
+                "sub.rn.f32 t, v01, v00;\n\t"
+                "fma.rn.f32 t, %6, t, v00;\n\t"
+                "sub.rn.f32 u, v11, v10;\n\t"
+                "fma.rn.f32 u, %6, u, v10;\n\t"
+                "sub.rn.f32 u, u, t;\n\t"
+                "fma.rn.f32 t, %7, u, t;\n\t"
+                "selp.f32 %0, t, 0f00000000, p;\n\t}"
+                : "=f"(phi)
+                : "r"(__float_as_uint(col)), "r"(cw_bits), "r"(__float_as_uint(row)), "r"(ch_bits), "r"(at), "f"(fx), "f"(fy),
+                  "r"(rpitch4));
+        }
         return phi;
     };
 
@@ -339,7 +370,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
 // The table's non-zero entries -> the IM column (S4).  kAtomic: the support was split into pieces, whose
 // contributions add up (linearity); the entries are cleared for the next piece.
 template <bool kAtomic, int NT>
-__device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_win, uint32_t tab_base,
+__device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_win, uint32_t tab_base, uint32_t krow_base,
                                               float *__restrict__ colp, int t0)
 {
     for (int w = 0; w < p.n_wfs; ++w) {
@@ -348,13 +379,10 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
         if (n <= 0) continue;
         const WfsDev &W = p.wfs[w];
         const uint32_t tb = tab_base + (uint32_t)W.tab_off * 4u;
-        const unsigned magic = 0xFFFFFFFFu / (unsigned)win.w + 1u;
         for (int e = t0; e < n; e += NT) {
             const float v = lds_f32(tb + (uint32_t)e * 4u);
             if (v == 0.0f) continue;
-            const int cell = e >> 1;
-            const int ra = win.w == 1 ? cell : (int)__umulhi((unsigned)cell, magic), rb = cell - ra * win.w;   // (magic wraps to 0 for 1)
-            const int k = __ldg(W.subap_row + (win.x + ra) * W.n_subap + (win.y + rb));
+            const int k = lds_s32(krow_base + (uint32_t)((W.tab_off >> 1) + (e >> 1)) * 4u);   // fetched while the strips ran
             if (k < 0) continue;
             float *dst = colp + ((e & 1) ? W.row_y : W.row_x) + k;
             if (kAtomic) {
@@ -367,10 +395,14 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
     }
 }
 
+// kCells: the staged pixels are turned into 16-byte bilinear cells first (supports small enough that the
+// cells leave six CTAs per SM); otherwise the four pixels of a sample are read from the staged box itself.
+template <bool kCells>
 __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
                                                                                      const __grid_constant__ CUtensorMap tmap)
 {
-    // [ raw TMA box: patch_pitch x patch_h floats | cells: cell_pitch x cell_h float4 | table: tab_floats ]
+    // [ raw TMA box: patch_pitch x patch_h floats | kCells: cell_pitch x cell_h float4 | table: tab_floats |
+    //   rows: tab_floats / 2 ints ]
     extern __shared__ __align__(128) float patch[];
     __shared__ __align__(8) uint64_t bar;
     __shared__ int4 s_win[kMaxWfsPerLaunch];
@@ -379,11 +411,19 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     float *colp = p.out + (long long)mode * p.ld;
     const uint32_t raw_base = smem_u32(patch);
     const uint32_t cell_base = raw_base + (uint32_t)(p.patch_pitch * p.patch_h) * 4u;   // patch_pitch % 4 == 0: 16-byte aligned
-    const uint32_t tab_base = cell_base + (uint32_t)(p.cell_pitch * p.cell_h) * 16u;
+    const uint32_t tab_base = cell_base + (kCells ? (uint32_t)(p.cell_pitch * p.cell_h) * 16u : 0u);
+    const uint32_t krow_base = tab_base + (uint32_t)p.tab_floats * 4u;   // IM row of each (a, b) of the windows
 
     const int4 b = __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode);
     const int bx0 = max(b.x, 0), by0 = max(b.y, 0), bx1 = min(b.z, p.nx - 1), by1 = min(b.w, p.ny - 1);
     const bool empty = bx1 < bx0 || by1 < by0;
+    // diagonal extents of the support: min/max of x+y and of x-y over its non-zero pixels (the bbox's own
+    // when the caller has none)
+    int sg0 = b.x + b.y, sg1 = b.z + b.w, dg0 = b.x - b.w, dg1 = b.z - b.y;
+    if (p.diag != nullptr) {
+        const int4 dg = __ldg(reinterpret_cast<const int4 *>(p.diag) + mode);
+        sg0 = max(sg0, dg.x); sg1 = min(sg1, dg.y); dg0 = max(dg0, dg.z); dg1 = min(dg1, dg.w);
+    }
 
     // pieces of the support that fit the staged box (one piece unless the bbox hint was too small).
     // Box layout: up to 3 columns of slack (the box must start on a 16-byte boundary of the source row),
@@ -401,17 +441,11 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
         mbar_expect_tx(&bar, box_bytes);
         tma_load_box(patch, &tmap, &bar, (bx0 - 1) & ~3, by0 - 1, mode);
     }
-    if (tid == 33 && p.prefetch_dist > 0 && mode + p.prefetch_dist < p.n_modes) {
-        // the box of a mode some CTAs ahead: DRAM latency under the column writes is long, L2 latency is not
-        const int4 nb = __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode + p.prefetch_dist);
-        if (nb.z >= nb.x && nb.w >= nb.y) tma_prefetch_box(&tmap, (max(nb.x, 0) - 1) & ~3, max(nb.y, 0) - 1, mode + p.prefetch_dist);
-    }
-    const uint32_t zbuf = tab_base + (uint32_t)p.tab_floats * 4u;   // p.zbuf_bytes of zeros, 16-byte aligned
-    for (int e = tid; e < p.tab_floats + (p.zbuf_bytes >> 2); e += kStripThreads) sts_f32(tab_base + (uint32_t)e * 4u, 0.0f);
+    for (int e = tid; e < p.tab_floats; e += kStripThreads) sts_f32(tab_base + (uint32_t)e * 4u, 0.0f);
     if (tid < kMaxWfsPerLaunch) s_win[tid] = make_int4(0, 0, 0, 0);
     // a split support adds into the column piece by piece: the zeros must be there first
     if (multi && p.zero_count > 0) zero_fill<kStripThreads>(colp + p.zero_begin, p.zero_count, tid);
-    __syncthreads();   // mbarrier initialised, table and zero buffer cleared
+    __syncthreads();   // mbarrier initialised, table cleared
 
     ZeroPacer zp;
     zp.v = nullptr; zp.left = 0;
@@ -435,13 +469,16 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             const int slack = qx0 - 1 - raw_x0;   // raw column `slack` is the left ring
             CellBox cb;
             cb.x0 = qx0 - 1; cb.y0 = qy0 - 1; cb.cw = qx1 - qx0 + 2; cb.ch = qy1 - qy0 + 2;
-            cb.base = cell_base; cb.pitch = p.cell_pitch;
+            cb.base = kCells ? cell_base : raw_base + (uint32_t)slack * 4u;
+            cb.pitch = kCells ? p.cell_pitch : p.patch_pitch;
+            cb.s_lo = (float)(sg0 - 2 - (cb.x0 + cb.y0)) - 0.01f; cb.s_hi = (float)(sg1 + 2 - (cb.x0 + cb.y0)) + 0.01f;
+            cb.d_lo = (float)(dg0 - 2 - (cb.x0 - cb.y0)) - 0.01f; cb.d_hi = (float)(dg1 + 2 - (cb.x0 - cb.y0)) + 0.01f;
             mbar_wait(&bar, parity);
             parity ^= 1u;
 
-            // raw pixels -> cells.  By linearity a piece is its own mode, zero outside its box: when the
-            // support was split, whatever the box holds on the piece's ring is read as 0.
-            {
+            // By linearity a piece is its own mode, zero outside its box: when the support was split, whatever
+            // the box holds on the piece's ring is read as 0.
+            if (kCells) {   // raw pixels -> cells
                 const int ncell = cb.cw * cb.ch;
                 const unsigned magic = 0xFFFFFFFFu / (unsigned)cb.cw + 1u;
                 const uint32_t rpitch4 = (uint32_t)p.patch_pitch * 4u;
@@ -460,30 +497,44 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                     const float dx = v01 - v00;
                     sts_f32x4(cell_base + (uint32_t)(r * p.cell_pitch + c) * 16u, make_float4(v00, dx, v10 - v00, (v11 - v10) - dx));
                 }
-            }
-            bar_sync(1, kComputeThreads);   // cells complete; the raw box is free again
-
-            if (pc + 1 < npieces && tid == 0) {   // next piece's box lands while this one is sampled
-                const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
-                fence_proxy_async();
-                mbar_expect_tx(&bar, box_bytes);
-                tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
+                bar_sync(1, kComputeThreads);   // cells complete; the raw box is free again
+                if (pc + 1 < npieces && tid == 0) {   // next piece's box lands while this one is sampled
+                    const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
+                    fence_proxy_async();
+                    mbar_expect_tx(&bar, box_bytes);
+                    tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
+                }
+            } else if (multi) {   // clear the ring just staged (pixels cw and ch are the far ring)
+                const uint32_t org = raw_base + (uint32_t)slack * 4u, rp4 = (uint32_t)p.patch_pitch * 4u;
+                for (int e = tid; e <= cb.cw; e += kComputeThreads) { sts_f32(org + (uint32_t)e * 4u, 0.0f); sts_f32(org + (uint32_t)cb.ch * rp4 + (uint32_t)e * 4u, 0.0f); }
+                for (int e = tid; e <= cb.ch; e += kComputeThreads) { sts_f32(org + (uint32_t)e * rp4, 0.0f); sts_f32(org + (uint32_t)e * rp4 + (uint32_t)cb.cw * 4u, 0.0f); }
+                bar_sync(1, kComputeThreads);
             }
 
             // lane w: footprint of this piece on sensor w.  phi(i,j) can be non-zero only strictly inside the
-            // image of the open box (qx0-1,qx1+1)x(qy0-1,qy1+1) under the inverse map, so D(i,j) only for
-            // floor(jmin) <= j <= ceil(jmax) (one pixel of stencil either side), clipped to the sensor
-            int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_nb = 0;
+            // image, under the inverse map, of the piece's open octagon: the box (qx0-1,qx1+1)x(qy0-1,qy1+1)
+            // cut by sg0-2 < x+y < sg1+2 and dg0-2 < x-y < dg1+2.  So D(i,j) only for floor(jmin) <= j <=
+            // ceil(jmax) (one pixel of stencil either side), clipped to the sensor.
+            int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_na = 0, r_nb = 0;
             if (lane < p.n_wfs) {
                 const WfsDev &W = p.wfs[lane];
+                const double X0 = qx0 - 1, X1 = qx1 + 1, Y0 = qy0 - 1, Y1 = qy1 + 1;
+                const double S0 = sg0 - 2, S1 = sg1 + 2, D0 = dg0 - 2, D1 = dg1 + 2;
                 double jmin = 1e300, jmax = -1e300, imin = 1e300, imax = -1e300;
-#pragma unroll
-                for (int cr = 0; cr < 4; ++cr) {
-                    const double c = (cr & 1) ? (double)(qx1 + 1) : (double)(qx0 - 1);
-                    const double r = (cr & 2) ? (double)(qy1 + 1) : (double)(qy0 - 1);
+                auto vertex = [&](double c, double r) {
                     const double j = W.inv[0] * c + W.inv[1] * r + W.inv[2];
                     const double i = W.inv[3] * c + W.inv[4] * r + W.inv[5];
                     jmin = fmin(jmin, j); jmax = fmax(jmax, j); imin = fmin(imin, i); imax = fmax(imax, i);
+                };
+                // two vertices on each edge of the box; an edge the diagonals cut away altogether yields two
+                // points outside the octagon but inside the box (a superset: still exact)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const double X = e ? X1 : X0, Y = e ? Y1 : Y0;
+                    const double ya = fmax(fmax(Y0, S0 - X), X - D1), yb = fmin(fmin(Y1, S1 - X), X - D0);
+                    vertex(X, ya); vertex(X, yb);
+                    const double xa = fmax(fmax(X0, S0 - Y), D0 + Y), xb = fmin(fmin(X1, S1 - Y), D1 + Y);
+                    vertex(xa, Y); vertex(xb, Y);
                 }
                 const double lim = 1.0e9;
                 r_j0 = max(0, (int)floor(fmax(jmin, -lim))); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)));
@@ -493,10 +544,22 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                     r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
                     r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
                     r_nb = r_j1 / W.n_pix - r_b0 + 1;
-                    win = make_int4(r_a0, r_b0, r_i1 / W.n_pix - r_a0 + 1, r_nb);
+                    r_na = r_i1 / W.n_pix - r_a0 + 1;
+                    win = make_int4(r_a0, r_b0, r_na, r_nb);
                     if (win.z * win.w * 2 > W.tab_cap) __trap();   // the host sized the table from the same bounds
                 }
                 if (warp == 0) s_win[lane] = win;   // read by scatter_table after a barrier
+            }
+            // the IM rows of the windows' subapertures, needed only when the table is stored: fetched now,
+            // asynchronously, so that the store at the end waits for nothing (sensor w by warp w mod 4)
+            for (int w = warp; w < p.n_wfs; w += kComputeWarps) {
+                const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
+                const int na = __shfl_sync(kFull, r_na, w);
+                const WfsDev &W = p.wfs[w];
+                for (int a = 0; a < na; ++a)
+                    for (int bq = lane; bq < nb; bq += 32)
+                        cp_async_4(krow_base + (uint32_t)((W.tab_off >> 1) + a * nb + bq) * 4u,
+                                   W.subap_row + (a0 + a) * W.n_subap + (b0 + bq));
             }
             int incl = r_n;
 #pragma unroll
@@ -513,30 +576,39 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                 const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
                 const int jA = j0 + (t - base) * kStripCols;
                 const int nC = min(kStripCols, j1 - jA + 1);
-                process_strip(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
+                process_strip<kCells>(p.wfs[w], i0, i1, jA, nC, cb, kCells ? p.addr_bias : p.addr_bias >> 2, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
             }
             if (multi) {
+                cp_async_wait_all();
                 bar_sync(1, kComputeThreads);   // every warp is done with these cells and this piece's table
-                scatter_table<true, kComputeThreads>(p, s_win, tab_base, colp, tid);
+                if (!kCells && pc + 1 < npieces && tid == 0) {   // the box itself was being sampled until now
+                    const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
+                    fence_proxy_async();
+                    mbar_expect_tx(&bar, box_bytes);
+                    tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
+                }
+                scatter_table<true, kComputeThreads>(p, s_win, tab_base, krow_base, colp, tid);
                 bar_sync(1, kComputeThreads);   // table clear again, windows free
             }
         }
     }
     while (zp.left > 0) zp.step();   // what the sampling loop did not get to
+    cp_async_wait_all();
     __syncthreads();                  // all zeros stored before anyone stores a value; table complete
-    if (!multi && npieces > 0) scatter_table<false, kStripThreads>(p, s_win, tab_base, colp, tid);
+    if (!multi && npieces > 0) scatter_table<false, kStripThreads>(p, s_win, tab_base, krow_base, colp, tid);
 }
 
 }  // namespace
 
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream)
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool cells, cudaStream_t stream)
 {
     if (p.n_modes <= 0) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(synim_strip_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    auto kernel = cells ? synim_strip_kernel<true> : synim_strip_kernel<false>;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     CUtensorMap tm;
     memcpy(&tm, tensor_map, sizeof(tm));
-    synim_strip_kernel<<<(unsigned)p.n_modes, kStripThreads, smem_bytes, stream>>>(p, tm);
+    kernel<<<(unsigned)p.n_modes, kStripThreads, smem_bytes, stream>>>(p, tm);
     return cudaGetLastError();
 }
 

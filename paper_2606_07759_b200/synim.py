@@ -72,10 +72,10 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).restype = i64
             getattr(L, name).argtypes = [vp, i32]
         L.synim_interaction_matrix.restype = ctypes.c_int
-        L.synim_interaction_matrix.argtypes = [vp, vp, i32, vp, i32, i32, ctypes.POINTER(WfsAffine), ctypes.c_int,
+        L.synim_interaction_matrix.argtypes = [vp, vp, i32, vp, vp, i32, i32, ctypes.POINTER(WfsAffine), ctypes.c_int,
                                                vp, i64, vp]
         L.synim_compute_bboxes.restype = ctypes.c_int
-        L.synim_compute_bboxes.argtypes = [vp, i32, i32, i32, vp, vp]
+        L.synim_compute_bboxes.argtypes = [vp, i32, i32, i32, vp, vp, vp]
         L.synim_bbox_extent.restype = ctypes.c_int
         L.synim_bbox_extent.argtypes = [vp, i32, ctypes.POINTER(i32), ctypes.POINTER(i32), vp]
         L.synim_interaction_matrix_host.restype = ctypes.c_int
@@ -193,12 +193,20 @@ def num_rows(geom: Geometry) -> int:
 
 def compute_bboxes(cube, stream=None):
     """Tight non-zero extents of a CUDA float32 cube [n][ny][nx] -> CUDA int32 [n][4]."""
+    return compute_supports(cube, stream, diagonals=False)[0]
+
+
+def compute_supports(cube, stream=None, diagonals=True):
+    """(bbox, diag): tight non-zero extents [n][4] and, if asked for, the diagonal extents
+    (min x+y, max x+y, min x-y, max x-y) [n][4] of every mode of a CUDA float32 cube [n][ny][nx]."""
     import torch
     assert cube.is_cuda and cube.dtype == torch.float32 and cube.is_contiguous() and cube.dim() == 3
     n, ny, nx = cube.shape
     out = torch.empty((n, 4), dtype=torch.int32, device=cube.device)
-    _check(lib().synim_compute_bboxes(cube.data_ptr(), n, ny, nx, out.data_ptr(), _stream_ptr(stream)))
-    return out
+    diag = torch.empty((n, 4), dtype=torch.int32, device=cube.device) if diagonals else None
+    _check(lib().synim_compute_bboxes(cube.data_ptr(), n, ny, nx, out.data_ptr(),
+                                      None if diag is None else diag.data_ptr(), _stream_ptr(stream)))
+    return out, diag
 
 
 def bbox_extent(bbox, stream=None):
@@ -211,7 +219,7 @@ def bbox_extent(bbox, stream=None):
 
 def interaction_matrix(geom: Geometry, cube, bbox, affines: Sequence[Sequence[float]],
                        scales: Optional[Sequence[float]] = None, out=None, bbox_max=(0, 0),
-                       mode: int = SLOPES_ND, stream=None):
+                       mode: int = SLOPES_ND, stream=None, diag=None):
     """synim_interaction_matrix on CUDA tensors.  Returns ``out`` viewed as [n_modes][ld] (row k of the
     view is IM column k: the buffer is the column-major IM)."""
     import torch
@@ -231,8 +239,12 @@ def interaction_matrix(geom: Geometry, cube, bbox, affines: Sequence[Sequence[fl
     if bbox is not None:
         assert bbox.is_cuda and bbox.dtype == torch.int32 and bbox.is_contiguous() and tuple(bbox.shape) == (n, 4)
         bptr = bbox.data_ptr()
+    dptr = None
+    if diag is not None:
+        assert diag.is_cuda and diag.dtype == torch.int32 and diag.is_contiguous() and tuple(diag.shape) == (n, 4)
+        dptr = diag.data_ptr()
     arr = _affine_array(affines, scales)
-    _check(lib().synim_interaction_matrix(geom._h, cube.data_ptr(), n, bptr, int(bbox_max[0]), int(bbox_max[1]),
+    _check(lib().synim_interaction_matrix(geom._h, cube.data_ptr(), n, bptr, dptr, int(bbox_max[0]), int(bbox_max[1]),
                                           arr, int(mode), out.data_ptr(), ld, _stream_ptr(stream)))
     return out
 

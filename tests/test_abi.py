@@ -63,7 +63,7 @@ def test_argument_errors_are_reported_not_thrown(lib):
     g = (synim.WfsGrid * 1)()
     assert lib.synim_create_geometry(8, 8, 0, g, None, ctypes.byref(h)) == synim.ERR_INVALID_ARG
     assert lib.synim_create_geometry(8, 10, 1, g, None, ctypes.byref(h)) == synim.ERR_ALIGNMENT
-    assert lib.synim_interaction_matrix(None, None, 1, None, 0, 0, None, 0, None, 1, None) == synim.ERR_INVALID_ARG
+    assert lib.synim_interaction_matrix(None, None, 1, None, None, 0, 0, None, 0, None, 1, None) == synim.ERR_INVALID_ARG
     w, hh = ctypes.c_int32(), ctypes.c_int32()
     assert lib.synim_bbox_extent(None, 0, ctypes.byref(w), ctypes.byref(hh), None) == synim.OK
 

@@ -28,14 +28,16 @@ def S():
     return synim
 
 
-def gpu_im(S, wl, affines=None, scales=None, use_bbox=True, ld_pad=0, hint=True):
+def gpu_im(S, wl, affines=None, scales=None, use_bbox=True, ld_pad=0, hint=True, octagon=True):
     """IM of a workload through the C ABI -> numpy float32 [rows][n_modes]."""
     import torch
     geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
     cube = torch.from_numpy(wl.cube).cuda()
-    bbox, bmax = None, (0, 0)
+    bbox, diag, bmax = None, None, (0, 0)
     if use_bbox and wl.bbox is not None:
         bbox = torch.from_numpy(wl.bbox).cuda()
+        if octagon:
+            diag = S.compute_supports(cube)[1]
         if hint:
             bmax = S.bbox_extent(bbox)
     rows = geom.num_rows
@@ -45,7 +47,7 @@ def gpu_im(S, wl, affines=None, scales=None, use_bbox=True, ld_pad=0, hint=True)
         affines = S.affines_of(wl)
     if scales is None:
         scales = [w.slope_scale for w in wl.wfs]
-    S.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax)
+    S.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax, diag=diag)
     torch.cuda.synchronize()
     res = out.cpu().numpy()
     if ld_pad:
@@ -200,7 +202,7 @@ def test_empty_and_degenerate_inputs(S):
         S.interaction_matrix(geom, cube, None, S.affines_of(wl), mode=S.SLOPES_GTILT)
     assert e.value.status == S.ERR_UNSUPPORTED
     small = torch.empty((wl.n_modes, geom.num_rows - 1), dtype=torch.float32, device="cuda")
-    assert S.lib().synim_interaction_matrix(geom._h, cube.data_ptr(), wl.n_modes, None, 0, 0,
+    assert S.lib().synim_interaction_matrix(geom._h, cube.data_ptr(), wl.n_modes, None, None, 0, 0,
                                             S._affine_array(S.affines_of(wl), None), 0, small.data_ptr(),
                                             geom.num_rows - 1, None) == S.ERR_INVALID_ARG
     geom.destroy()
@@ -238,6 +240,29 @@ def test_compute_bboxes_matches_the_generator(S):
     exp = W.tight_bboxes(wl.cube)
     assert np.array_equal(got.cpu().numpy(), exp)
     assert S.bbox_extent(got) == (int((exp[:, 2] - exp[:, 0] + 1).max()), int((exp[:, 3] - exp[:, 1] + 1).max()))
+    # diagonal extents: min/max of x+y and x-y over the non-zero pixels, written out with numpy
+    bb, dg = S.compute_supports(torch.from_numpy(wl.cube).cuda())
+    assert np.array_equal(bb.cpu().numpy(), exp)
+    dg = dg.cpu().numpy()
+    for m in range(wl.n_modes):
+        yy, xx = np.nonzero(wl.cube[m])
+        want = (0, -1, 0, -1) if len(xx) == 0 else ((xx + yy).min(), (xx + yy).max(), (xx - yy).min(), (xx - yy).max())
+        assert tuple(int(v) for v in dg[m]) == tuple(int(v) for v in want), m
+
+
+def test_octagon_footprints_change_nothing_but_the_work(S):
+    """The diagonal extents only narrow what is sampled: same IM with and without them, on rotated
+    sensors (config 3) and on the split-support path (no size hint, config 4's 60-pixel supports)."""
+    wl = W.make_config(3, max_modes=96)
+    a = gpu_im(S, wl, octagon=True)
+    b = gpu_im(S, wl, octagon=False)
+    ref = O.interaction_matrix(wl)
+    assert_parity(a, ref, wl)
+    assert_parity(b, ref, wl)
+    scale = np.abs(ref).max()
+    assert np.abs(a.astype(np.float64) - b.astype(np.float64)).max() <= 1e-6 * scale
+    wl = W.make_config(4, max_modes=24)
+    assert_parity(gpu_im(S, wl, octagon=True, hint=False), O.interaction_matrix(wl), wl)
 
 
 def test_host_buffer_entry_point(S):

@@ -367,8 +367,6 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     }
     const int phi_h = tile_cap + 2;
     const int phi_pitch = (tile_cap + 2) | 1;   // odd pitch: rows of a subaperture fall in different banks
-    // strip kernel: one float4 bilinear cell per pixel pair of (piece + ring) behind the raw TMA box
-    const int cell_pitch = patch_pitch - 5 + 1, cell_h = patch_h - 2 + 1;
     // strip kernel: per sensor a table of (x, y) partial slopes over the window of subapertures one
     // piece's footprint can span (the kernel derives the window from the same bounds and traps if it
     // ever needed more)
@@ -392,13 +390,9 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
             tab_floats_max = std::max(tab_floats_max, (off + 3) & ~3);
         }
     }
-    // bilinear cells only while they leave six CTAs per SM (what the registers allow): 228 KB / 6 - 1 KB each
-    const size_t strip_fixed = sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)tab_floats_max) +
-                               sizeof(int) * (size_t)(tab_floats_max / 2);
-    const size_t strip_cells = sizeof(float) * 4 * (size_t)cell_pitch * cell_h;
-    const bool use_cells = !dense && strip_fixed + strip_cells <= (228 * 1024) / 6 - 1024 && !getenv("SYNIM_NOCELLS");   // TEMP env
     const size_t smem = dense ? sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)phi_pitch * phi_h)
-                              : strip_fixed + (use_cells ? strip_cells : 0);
+                              : sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)tab_floats_max) +
+                                    sizeof(int) * (size_t)(tab_floats_max / 2);
     CUtensorMap tmap;
     if (!dense) {
         synim_status st = encode_cube_map(d_influence, n_modes, ny, nx, patch_pitch, patch_h, &tmap);
@@ -419,8 +413,7 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         std::memset(&p, 0, sizeof(p));
         p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.out = d_out; p.ld = ld;
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
-        p.addr_bias = 0x4B400000u << 4;
-        p.cell_pitch = cell_pitch; p.cell_h = cell_h;
+        p.addr_bias = 0x4B400000u << 2;
         p.patch_pitch = patch_pitch; p.patch_h = patch_h; p.phi_pitch = phi_pitch; p.phi_h = phi_h;
         for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
         p.tab_floats = nw > 0 ? (dev[w0 + nw - 1].tab_off + dev[w0 + nw - 1].tab_cap + 3) & ~3 : 0;
@@ -436,7 +429,7 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
             p.jobs_per_mode = 1;
         }
         if (dense) SYNIM_CUDA(synim::launch_interaction_matrix(p, smem, s));
-        else SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, use_cells, s));
+        else SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));
     }
     return SYNIM_OK;
 }

@@ -44,8 +44,7 @@ struct ImParams {
                                 // by the mode's CTA before it accumulates (0: caller pre-zeroed)
     int jobs_per_mode;          // 1: one CTA per mode walks every sensor; else n_wfs*chunks CTAs per mode
     int chunks;                 // tile chunks per sensor when jobs_per_mode > 1
-    unsigned addr_bias;         // strip kernel: (bits of 1.5*2^23) << 4 mod 2^32, see process_strip
-    int cell_pitch, cell_h;     // strip kernel: capacity of the bilinear-cell array (float4 cells)
+    unsigned addr_bias;         // strip kernel: (bits of 1.5*2^23) << 2 mod 2^32, see process_strip
     int tab_floats;             // strip kernel: size of the CTA's slope table (multiple of 4)
     WfsDev wfs[kMaxWfsPerLaunch];
 };
@@ -53,8 +52,8 @@ struct ImParams {
 // launchers (synim_kernels.cu); all asynchronous on `stream`, return the launch status
 cudaError_t launch_interaction_matrix(const ImParams &p, size_t smem_bytes, cudaStream_t stream);
 // compact-support path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
-// {patch_pitch, patch_h, 1}; cells: build 16-byte bilinear cells from the staged box (smem_bytes covers them)
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool cells, cudaStream_t stream);
+// {patch_pitch, patch_h, 1}
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
                                  float *d_wmap, int *d_error_flag, cudaStream_t stream);
 cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox, int *d_diag,

@@ -3,25 +3,27 @@
 // One CTA per mode.  The mode's support (its bbox plus the one-pixel ring a bilinear sample can still
 // touch) is staged ONCE in shared memory by a TMA 3-D box load (cp.async.bulk.tensor, out-of-range
 // elements zero-filled by the hardware = reading R4) and reused by every sensor of the batch
-// (the cube is fetched once for all WFS).  While the load is in flight the CTA streams
-// the zeros of its whole IM column (S4).  The staged pixels are then turned, once, into bilinear
-// CELLS (v00, v01-v00, v10-v00, v11-v10-v01+v00), so that a sample is one 16-byte LDS and three FFMA.
-// Then each warp takes "strips": 30 WFS pixel columns (one per lane, plus one halo column on either
-// side) of one sensor's footprint, and walks down the pixel rows two at a time, keeping phi of the
-// previous two rows in registers:
+// (the cube is fetched once for all WFS).  Each warp then takes "strips": 30 WFS pixel
+// columns (one per lane, plus one halo column on either side) of one sensor's footprint -- the image of
+// the support's bounding OCTAGON under the inverse map -- and walks down the pixel rows, keeping phi
+// of the previous two rows in registers:
 //   S1  col/row = tile-local float32 offsets from a float64 per-lane base,
 //   S2  floor/fraction with the 1.5*2^23 trick, the shared-memory address straight from the float
-//       mantissa, one LDS.128 + 3 FFMA per sample; a sample outside the staged box is 0 (R4, R15),
+//       mantissa, 4 predicated LDS + 3 lerps per sample, branch-free; a sample outside the staged box
+//       is 0 (R4, R15),
 //   S3  D_y from registers, D_x from the two neighbouring lanes (shuffles), weighted by the
-//       precomputed 0.5*P/W_S map, summed down the rows of a subaperture in registers and across
-//       its columns with a segmented warp-shuffle reduction,
-//   S4  one float add into the (already zeroed) column per (subaperture, axis).
+//       precomputed 0.5*P/W_S map, summed down the rows of a subaperture in registers, across its
+//       columns with a segmented warp-shuffle reduction, and into a per-CTA shared table of
+//       (sensor, subaperture, axis) slopes,
+//   S4  the column is written once: its zeros by plain 16-byte stores PACED through the sampling loop
+//       (one per thread per iteration), then the table's non-zero entries on top.
 // Rows of a strip that cannot touch the support are never sampled (exact: phi is 0 there, R15).
 // phi is never written anywhere.
 //
-// Measured on B200 (_work microbenchmarks, round 1): FFMA2/FADD2 occupy the issue port for two cycles,
-// so packing pixel pairs into f32x2 saves nothing in an issue-bound kernel; LDS and SHFL each run at
-// about one warp instruction per clock per SM.  Hence scalar FP32 and as few LDS as possible.
+// Measured on B200, round 1 (profiles/README.md): FFMA2/FADD2 occupy the issue port for two cycles, so
+// packing pixel pairs into f32x2 saves nothing; LDS and SHFL each run at about one warp instruction
+// per clock per SM; and dumping a CTA's 161 KB of zeros in one go (plain stores, TMA bulk copies, or
+// a warp of its own) delays every load of the SM behind the store data -- hence the pacing.
 #include "synim_device.h"
 
 #include <cstring>
@@ -34,15 +36,10 @@ namespace {
 constexpr int kComputeWarps = 4, kComputeThreads = 32 * kComputeWarps;
 constexpr int kStripThreads = kComputeThreads;
 #ifndef SYNIM_STRIP_MINB
-#define SYNIM_STRIP_MINB 6
-#endif
-#ifdef SYNIM_EXP_NOW   // TEMP experiment: no weight loads
-#define SYNIM_WLOAD(p) (isD ? 0.01f : 0.0f)
-#else
-#define SYNIM_WLOAD(p) __ldg(p)
+#define SYNIM_STRIP_MINB 7
 #endif
 #ifndef SYNIM_STRIP_ROWS
-#define SYNIM_STRIP_ROWS 4
+#define SYNIM_STRIP_ROWS 2
 #endif
 constexpr int kStripRows = SYNIM_STRIP_ROWS;                // pixel rows per loop iteration (independent samples in flight per lane)
 static_assert(2 * kStripRows <= kWmapPadRows, "weight look-ahead runs past the rows of zeros");
@@ -113,11 +110,6 @@ __device__ __forceinline__ void red_shared_f32(uint32_t addr, float v)
 }
 __device__ __forceinline__ void sts_f32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
 __device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
-__device__ __forceinline__ void sts_f32x4(uint32_t addr, float4 v)
-{
-    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
-}
-
 template <int NT>
 __device__ __forceinline__ void zero_fill(float *dst, int n, int tid)
 {
@@ -134,14 +126,14 @@ __device__ __forceinline__ void zero_fill(float *dst, int n, int tid)
     if (tid < n - done) dst[done + tid] = 0.0f;
 }
 
-// The bilinear cells of one staged piece.  Cell (r, c) covers source pixels x0+c .. x0+c+1, y0+r .. y0+r+1,
-// where (x0, y0) is the upper-left pixel of the piece's ring of zeros; a sample at (col, row) relative to
-// (x0, y0) can be non-zero only for 0 <= col < cw, 0 <= row < ch.
+// One staged piece.  Cell (r, c) covers source pixels x0+c .. x0+c+1, y0+r .. y0+r+1, where (x0, y0) is
+// the upper-left pixel of the piece's ring of zeros; a sample at (col, row) relative to (x0, y0) can be
+// non-zero only for 0 <= col < cw, 0 <= row < ch.
 struct CellBox {
     int x0, y0;      // absolute source pixel of cell (0, 0)
     int cw, ch;      // cells per row / rows of cells: piece width + 1, piece height + 1
-    uint32_t base;   // shared-window byte address of cell (0, 0), or of its upper-left pixel in the raw box
-    int pitch;       // cells (or pixels) per row of the array
+    uint32_t base;   // shared-window byte address of pixel (x0, y0) in the staged box
+    int pitch;       // floats per row of the staged box
     // a sample can be non-zero only for s_lo < col+row < s_hi and d_lo < col-row < d_hi as well (the
     // support's bounding octagon, grown by the reach of a bilinear sample)
     float s_lo, s_hi, d_lo, d_hi;
@@ -174,7 +166,6 @@ struct ZeroPacer {
 // One strip: D columns jA .. jA+nC-1 (lanes 1..nC), D rows i0 .. i1 of sensor W.
 // Its partial slopes are added to the CTA's shared table: entry (a, b, axis) of the sensor's window of
 // subapertures (first row a0, first column b0, nb columns) sits at tab + ((a-a0)*nb + (b-b0))*8 + axis*4.
-template <bool kCells>
 __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
                                               uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp)
 {
@@ -262,15 +253,14 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         tent += tstep;
     };
 
-    // S2: one bilinear sample of phi row rf from the cells; 0 outside them.  Non-negative floats order like
+    // S2: one bilinear sample of phi row rf from the staged pixels; 0 outside them.  Non-negative floats order like
     // their bit patterns and negative ones have the sign bit set, so one unsigned compare per axis
     // tests 0 <= x < limit.  Branch-free (predicated LDS), so that the kRows samples of an iteration
     // overlap: the kernel is latency-bound otherwise (ncu, round 1).
     const uint32_t cw_bits = __float_as_uint(cwf), ch_bits = __float_as_uint(chf);
     const float pitchf = (float)cb.pitch;
-    // byte address of element 0 minus (bits of the magic number << 4, or << 2 for pixels) mod 2^32.  The
-    // bias is a kernel parameter, not a literal, so that ptxas keeps the difference in one register and
-    // an address is one LEA
+    // byte address of element 0 minus (bits of the magic number << 2) mod 2^32.  The bias is a kernel
+    // parameter, not a literal, so that ptxas keeps the difference in one register and an address is one LEA
     const uint32_t cbase = cb.base - addr_bias;
     const uint32_t rpitch4 = (uint32_t)cb.pitch * 4u;
     auto sample = [&](float rf) -> float {
@@ -279,42 +269,27 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         const float fx = col - (tc - kMagicFloor), fy = row - (tr - kMagicFloor);
         // magic + c0 + r0*pitch is exact: its mantissa is the element index
         const uint32_t idx = __float_as_uint(fmaf(tr - kMagicFloor, pitchf, tc));
+        const uint32_t at = idx * 4u + cbase;
         float phi;
-        if (kCells) {   // one 16-byte cell: v00, v01-v00, v10-v00, v11-v10-v01+v00
-            const uint32_t at = idx * 16u + cbase;
-            asm volatile(
-                "{\n\t.reg .pred p;\n\t.reg .f32 v, gx, gy, gxy, t;\n\t"
-                "setp.lt.u32 p, %1, %2;\n\t"
-                "setp.lt.and.u32 p, %3, %4, p;\n\t"
-                "@p ld.shared.v4.f32 {v, gx, gy, gxy}, [%5];\n\t"
-                "fma.rn.f32 t, %6, gxy, gy;\n\t"
-                "fma.rn.f32 t, %7, t, v;\n\t"
-                "fma.rn.f32 t, %6, gx, t;\n\t"
-                "selp.f32 %0, t, 0f00000000, p;\n\t}"
-                : "=f"(phi)
-                : "r"(__float_as_uint(col)), "r"(cw_bits), "r"(__float_as_uint(row)), "r"(ch_bits), "r"(at), "f"(fx), "f"(fy));
-        } else {        // the four pixels straight from the staged box (supports too large for cells)
-            const uint32_t at = idx * 4u + cbase;
-            asm volatile(
-                "{\n\t.reg .pred p;\n\t.reg .f32 v00, v01, v10, v11, t, u;\n\t.reg .b32 at1;\n\t"
-                "setp.lt.u32 p, %1, %2;\n\t"
-                "setp.lt.and.u32 p, %3, %4, p;\n\t"
-                "add.u32 at1, %5, %8;\n\t"
-                "@p ld.shared.f32 v00, [%5];\n\t"
-                "@p ld.shared.f32 v01, [%5+4];\n\t"
-                "@p ld.shared.f32 v10, [at1];\n\t"
-                "@p ld.shared.f32 v11, [at1+4];\n\t"
-                "sub.rn.f32 t, v01, v00;\n\t"
-                "fma.rn.f32 t, %6, t, v00;\n\t"
-                "sub.rn.f32 u, v11, v10;\n\t"
-                "fma.rn.f32 u, %6, u, v10;\n\t"
-                "sub.rn.f32 u, u, t;\n\t"
-                "fma.rn.f32 t, %7, u, t;\n\t"
-                "selp.f32 %0, t, 0f00000000, p;\n\t}"
-                : "=f"(phi)
-                : "r"(__float_as_uint(col)), "r"(cw_bits), "r"(__float_as_uint(row)), "r"(ch_bits), "r"(at), "f"(fx), "f"(fy),
-                  "r"(rpitch4));
-        }
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t.reg .f32 v00, v01, v10, v11, t, u;\n\t.reg .b32 at1;\n\t"
+            "setp.lt.u32 p, %1, %2;\n\t"
+            "setp.lt.and.u32 p, %3, %4, p;\n\t"
+            "add.u32 at1, %5, %8;\n\t"
+            "@p ld.shared.f32 v00, [%5];\n\t"
+            "@p ld.shared.f32 v01, [%5+4];\n\t"
+            "@p ld.shared.f32 v10, [at1];\n\t"
+            "@p ld.shared.f32 v11, [at1+4];\n\t"
+            "sub.rn.f32 t, v01, v00;\n\t"
+            "fma.rn.f32 t, %6, t, v00;\n\t"
+            "sub.rn.f32 u, v11, v10;\n\t"
+            "fma.rn.f32 u, %6, u, v10;\n\t"
+            "sub.rn.f32 u, u, t;\n\t"
+            "fma.rn.f32 t, %7, u, t;\n\t"
+            "selp.f32 %0, t, 0f00000000, p;\n\t}"
+            : "=f"(phi)
+            : "r"(__float_as_uint(col)), "r"(cw_bits), "r"(__float_as_uint(row)), "r"(ch_bits), "r"(at), "f"(fx), "f"(fy),
+              "r"(rpitch4));
         return phi;
     };
 
@@ -323,7 +298,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     float pmA = sample((float)(d_lo - 1)), pmB = sample((float)d_lo);   // phi[d-1], phi[d]
     float wgt[kRows];
 #pragma unroll
-    for (int k = 0; k < kRows; ++k) wgt[k] = SYNIM_WLOAD(S.wmap + (woff + (uint32_t)k * wrow));
+    for (int k = 0; k < kRows; ++k) wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
     float sx = 0.0f, sy = 0.0f;
 #pragma unroll 1
     for (int d = d_lo; d <= d_hi; d += kRows) {
@@ -332,7 +307,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         woff += wstride;
         float wnx[kRows];
 #pragma unroll
-        for (int k = 0; k < kRows; ++k) wnx[k] = SYNIM_WLOAD(S.wmap + (woff + (uint32_t)k * wrow));
+        for (int k = 0; k < kRows; ++k) wnx[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
 
         float cur[kRows];   // phi[d+1 .. d+kRows]
 #pragma unroll
@@ -395,14 +370,10 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
     }
 }
 
-// kCells: the staged pixels are turned into 16-byte bilinear cells first (supports small enough that the
-// cells leave six CTAs per SM); otherwise the four pixels of a sample are read from the staged box itself.
-template <bool kCells>
 __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
                                                                                      const __grid_constant__ CUtensorMap tmap)
 {
-    // [ raw TMA box: patch_pitch x patch_h floats | kCells: cell_pitch x cell_h float4 | table: tab_floats |
-    //   rows: tab_floats / 2 ints ]
+    // [ TMA box: patch_pitch x patch_h floats | table: tab_floats | rows: tab_floats / 2 ints ]
     extern __shared__ __align__(128) float patch[];
     __shared__ __align__(8) uint64_t bar;
     __shared__ int4 s_win[kMaxWfsPerLaunch];
@@ -410,8 +381,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     const int mode = blockIdx.x;
     float *colp = p.out + (long long)mode * p.ld;
     const uint32_t raw_base = smem_u32(patch);
-    const uint32_t cell_base = raw_base + (uint32_t)(p.patch_pitch * p.patch_h) * 4u;   // patch_pitch % 4 == 0: 16-byte aligned
-    const uint32_t tab_base = cell_base + (kCells ? (uint32_t)(p.cell_pitch * p.cell_h) * 16u : 0u);
+    const uint32_t tab_base = raw_base + (uint32_t)(p.patch_pitch * p.patch_h) * 4u;
     const uint32_t krow_base = tab_base + (uint32_t)p.tab_floats * 4u;   // IM row of each (a, b) of the windows
 
     const int4 b = __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode);
@@ -469,8 +439,8 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             const int slack = qx0 - 1 - raw_x0;   // raw column `slack` is the left ring
             CellBox cb;
             cb.x0 = qx0 - 1; cb.y0 = qy0 - 1; cb.cw = qx1 - qx0 + 2; cb.ch = qy1 - qy0 + 2;
-            cb.base = kCells ? cell_base : raw_base + (uint32_t)slack * 4u;
-            cb.pitch = kCells ? p.cell_pitch : p.patch_pitch;
+            cb.base = raw_base + (uint32_t)slack * 4u;
+            cb.pitch = p.patch_pitch;
             cb.s_lo = (float)(sg0 - 2 - (cb.x0 + cb.y0)) - 0.01f; cb.s_hi = (float)(sg1 + 2 - (cb.x0 + cb.y0)) + 0.01f;
             cb.d_lo = (float)(dg0 - 2 - (cb.x0 - cb.y0)) - 0.01f; cb.d_hi = (float)(dg1 + 2 - (cb.x0 - cb.y0)) + 0.01f;
             mbar_wait(&bar, parity);
@@ -478,33 +448,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
 
             // By linearity a piece is its own mode, zero outside its box: when the support was split, whatever
             // the box holds on the piece's ring is read as 0.
-            if (kCells) {   // raw pixels -> cells
-                const int ncell = cb.cw * cb.ch;
-                const unsigned magic = 0xFFFFFFFFu / (unsigned)cb.cw + 1u;
-                const uint32_t rpitch4 = (uint32_t)p.patch_pitch * 4u;
-                for (int e = tid; e < ncell; e += kComputeThreads) {
-                    const int r = (int)__umulhi((unsigned)e, magic);
-                    const int c = e - r * cb.cw;
-                    const uint32_t at = raw_base + (uint32_t)(r * p.patch_pitch + slack + c) * 4u;
-                    float v00 = lds_f32(at), v01 = lds_f32(at + 4u), v10 = lds_f32(at + rpitch4), v11 = lds_f32(at + rpitch4 + 4u);
-                    if (multi) {
-                        const bool l = c == 0, rgt = c == cb.cw - 1, t = r == 0, bt = r == cb.ch - 1;
-                        if (l || t) v00 = 0.0f;
-                        if (rgt || t) v01 = 0.0f;
-                        if (l || bt) v10 = 0.0f;
-                        if (rgt || bt) v11 = 0.0f;
-                    }
-                    const float dx = v01 - v00;
-                    sts_f32x4(cell_base + (uint32_t)(r * p.cell_pitch + c) * 16u, make_float4(v00, dx, v10 - v00, (v11 - v10) - dx));
-                }
-                bar_sync(1, kComputeThreads);   // cells complete; the raw box is free again
-                if (pc + 1 < npieces && tid == 0) {   // next piece's box lands while this one is sampled
-                    const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
-                    fence_proxy_async();
-                    mbar_expect_tx(&bar, box_bytes);
-                    tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
-                }
-            } else if (multi) {   // clear the ring just staged (pixels cw and ch are the far ring)
+            if (multi) {   // clear the ring just staged (pixels cw and ch are the far ring)
                 const uint32_t org = raw_base + (uint32_t)slack * 4u, rp4 = (uint32_t)p.patch_pitch * 4u;
                 for (int e = tid; e <= cb.cw; e += kComputeThreads) { sts_f32(org + (uint32_t)e * 4u, 0.0f); sts_f32(org + (uint32_t)cb.ch * rp4 + (uint32_t)e * 4u, 0.0f); }
                 for (int e = tid; e <= cb.ch; e += kComputeThreads) { sts_f32(org + (uint32_t)e * rp4, 0.0f); sts_f32(org + (uint32_t)e * rp4 + (uint32_t)cb.cw * 4u, 0.0f); }
@@ -576,12 +520,12 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                 const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
                 const int jA = j0 + (t - base) * kStripCols;
                 const int nC = min(kStripCols, j1 - jA + 1);
-                process_strip<kCells>(p.wfs[w], i0, i1, jA, nC, cb, kCells ? p.addr_bias : p.addr_bias >> 2, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
+                process_strip(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
             }
             if (multi) {
                 cp_async_wait_all();
-                bar_sync(1, kComputeThreads);   // every warp is done with these cells and this piece's table
-                if (!kCells && pc + 1 < npieces && tid == 0) {   // the box itself was being sampled until now
+                bar_sync(1, kComputeThreads);   // every warp is done with this box and this piece's table
+                if (pc + 1 < npieces && tid == 0) {   // the box was being sampled until now
                     const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
                     fence_proxy_async();
                     mbar_expect_tx(&bar, box_bytes);
@@ -600,15 +544,14 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
 
 }  // namespace
 
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool cells, cudaStream_t stream)
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream)
 {
     if (p.n_modes <= 0) return cudaSuccess;
-    auto kernel = cells ? synim_strip_kernel<true> : synim_strip_kernel<false>;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    cudaError_t e = cudaFuncSetAttribute(synim_strip_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     CUtensorMap tm;
     memcpy(&tm, tensor_map, sizeof(tm));
-    kernel<<<(unsigned)p.n_modes, kStripThreads, smem_bytes, stream>>>(p, tm);
+    synim_strip_kernel<<<(unsigned)p.n_modes, kStripThreads, smem_bytes, stream>>>(p, tm);
     return cudaGetLastError();
 }
 

@@ -300,8 +300,9 @@ def main():
                                                                        float(per_step.max())]}),
                 "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                              "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                             "algorithmic_bytes": ab, "kernel": "synim_im_kernel", "kernel_ms": kernel_ms},
-                "clocks": clocks, "gpu_launches": args.steps * (1 if wl.bbox is not None else 1),
+                             "algorithmic_bytes": ab, "kernel": "synim_strip_kernel" if wl.bbox is not None else "synim_im_kernel",
+                             "kernel_ms": kernel_ms},
+                "clocks": clocks, "gpu_launches": args.steps * ((len(wl.wfs) + 15) // 16),
                 "parity_spot_check": parity}
         if e2e:
             line["e2e"] = {"value": plan["total_units"] / (e2e_ms * 1e-3), "unit": UNIT,

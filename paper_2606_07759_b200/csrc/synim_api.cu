@@ -414,6 +414,7 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.out = d_out; p.ld = ld;
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
         p.addr_bias = 0x4B400000u << 2;
+        p.patch_pitchf = (float)patch_pitch;
         p.patch_pitch = patch_pitch; p.patch_h = patch_h; p.phi_pitch = phi_pitch; p.phi_h = phi_h;
         for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
         p.tab_floats = nw > 0 ? (dev[w0 + nw - 1].tab_off + dev[w0 + nw - 1].tab_cap + 3) & ~3 : 0;

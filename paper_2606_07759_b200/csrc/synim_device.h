@@ -44,6 +44,7 @@ struct ImParams {
                                 // by the mode's CTA before it accumulates (0: caller pre-zeroed)
     int jobs_per_mode;          // 1: one CTA per mode walks every sensor; else n_wfs*chunks CTAs per mode
     int chunks;                 // tile chunks per sensor when jobs_per_mode > 1
+    float patch_pitchf;         // strip kernel: patch_pitch as float (an FFMA operand straight from constant memory)
     unsigned addr_bias;         // strip kernel: (bits of 1.5*2^23) << 2 mod 2^32, see process_strip
     int tab_floats;             // strip kernel: size of the CTA's slope table (multiple of 4)
     WfsDev wfs[kMaxWfsPerLaunch];

@@ -134,6 +134,7 @@ struct CellBox {
     int cw, ch;      // cells per row / rows of cells: piece width + 1, piece height + 1
     uint32_t base;   // shared-window byte address of pixel (x0, y0) in the staged box
     int pitch;       // floats per row of the staged box
+    float pitchf;    // the same, as float
     // a sample can be non-zero only for s_lo < col+row < s_hi and d_lo < col-row < d_hi as well (the
     // support's bounding octagon, grown by the reach of a bilinear sample)
     float s_lo, s_hi, d_lo, d_hi;
@@ -151,16 +152,17 @@ struct StripSensor {
 // copies, or a warp of its own: all measured -- fills the SM's path to L2, and every load of the other
 // warps then waits behind 161 KB of store data.)
 struct ZeroPacer {
-    float4 *v;   // the thread's next piece
-    int left;    // pieces this thread still has to write
+    float4 *base;    // first 16-byte piece of the column (CTA-uniform)
+    uint32_t next;   // the thread's next piece
+    uint32_t end;    // number of pieces
     __device__ __forceinline__ void step()
     {
-        if (left > 0) {
-            *v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-            v += kStripThreads;
-            --left;
+        if (next < end) {
+            base[next] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            next += kStripThreads;
         }
     }
+    __device__ __forceinline__ bool pending() const { return next < end; }
 };
 
 // One strip: D columns jA .. jA+nC-1 (lanes 1..nC), D rows i0 .. i1 of sensor W.
@@ -258,7 +260,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // tests 0 <= x < limit.  Branch-free (predicated LDS), so that the kRows samples of an iteration
     // overlap: the kernel is latency-bound otherwise (ncu, round 1).
     const uint32_t cw_bits = __float_as_uint(cwf), ch_bits = __float_as_uint(chf);
-    const float pitchf = (float)cb.pitch;
+    const float pitchf = cb.pitchf;
     // byte address of element 0 minus (bits of the magic number << 2) mod 2^32.  The bias is a kernel
     // parameter, not a literal, so that ptxas keeps the difference in one register and an address is one LEA
     const uint32_t cbase = cb.base - addr_bias;
@@ -377,6 +379,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     extern __shared__ __align__(128) float patch[];
     __shared__ __align__(8) uint64_t bar;
     __shared__ int4 s_win[kMaxWfsPerLaunch];
+    __shared__ int s_next;   // next strip of the current piece
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int mode = blockIdx.x;
     float *colp = p.out + (long long)mode * p.ld;
@@ -413,12 +416,13 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     }
     for (int e = tid; e < p.tab_floats; e += kStripThreads) sts_f32(tab_base + (uint32_t)e * 4u, 0.0f);
     if (tid < kMaxWfsPerLaunch) s_win[tid] = make_int4(0, 0, 0, 0);
+    if (tid == 0) s_next = 0;
     // a split support adds into the column piece by piece: the zeros must be there first
     if (multi && p.zero_count > 0) zero_fill<kStripThreads>(colp + p.zero_begin, p.zero_count, tid);
     __syncthreads();   // mbarrier initialised, table cleared
 
     ZeroPacer zp;
-    zp.v = nullptr; zp.left = 0;
+    zp.base = nullptr; zp.next = 0; zp.end = 0;
     if (!multi && p.zero_count > 0) {
         float *z = colp + p.zero_begin;
         const int mis = (int)((reinterpret_cast<uintptr_t>(z) >> 2) & 3);
@@ -426,8 +430,8 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
         const int body = (p.zero_count - headn) >> 2, tailn = p.zero_count - headn - (body << 2);
         if (tid < headn) z[tid] = 0.0f;
         if (tid < tailn) z[headn + (body << 2) + tid] = 0.0f;
-        zp.v = reinterpret_cast<float4 *>(z + headn) + tid;
-        zp.left = (body - tid + kStripThreads - 1) / kStripThreads;
+        zp.base = reinterpret_cast<float4 *>(z + headn);
+        zp.next = (uint32_t)tid; zp.end = (uint32_t)body;
     }
     {
         uint32_t parity = 0;
@@ -441,6 +445,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             cb.x0 = qx0 - 1; cb.y0 = qy0 - 1; cb.cw = qx1 - qx0 + 2; cb.ch = qy1 - qy0 + 2;
             cb.base = raw_base + (uint32_t)slack * 4u;
             cb.pitch = p.patch_pitch;
+            cb.pitchf = p.patch_pitchf;
             cb.s_lo = (float)(sg0 - 2 - (cb.x0 + cb.y0)) - 0.01f; cb.s_hi = (float)(sg1 + 2 - (cb.x0 + cb.y0)) + 0.01f;
             cb.d_lo = (float)(dg0 - 2 - (cb.x0 - cb.y0)) - 0.01f; cb.d_hi = (float)(dg1 + 2 - (cb.x0 - cb.y0)) + 0.01f;
             mbar_wait(&bar, parity);
@@ -512,7 +517,13 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                 if (lane >= d) incl += t;
             }
             const int total = __shfl_sync(kFull, incl, 31);
-            for (int t = warp; t < total; t += kComputeWarps) {
+            // strips are handed out first come, first served: their costs differ (a strip over the rim of a
+            // round support has fewer live rows), and the CTA ends with its slowest warp
+            while (true) {
+                int t = 0;
+                if (lane == 0) t = atomicAdd(&s_next, 1);
+                t = __shfl_sync(kFull, t, 0);
+                if (t >= total) break;
                 const int w = __popc(__ballot_sync(kFull, incl <= t));
                 const int base = __shfl_sync(kFull, incl - r_n, w);
                 const int i0 = __shfl_sync(kFull, r_i0, w), i1 = __shfl_sync(kFull, r_i1, w);
@@ -532,11 +543,12 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                     tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
                 }
                 scatter_table<true, kComputeThreads>(p, s_win, tab_base, krow_base, colp, tid);
+                if (tid == 0) s_next = 0;
                 bar_sync(1, kComputeThreads);   // table clear again, windows free
             }
         }
     }
-    while (zp.left > 0) zp.step();   // what the sampling loop did not get to
+    while (zp.pending()) zp.step();   // what the sampling loop did not get to
     cp_async_wait_all();
     __syncthreads();                  // all zeros stored before anyone stores a value; table complete
     if (!multi && npieces > 0) scatter_table<false, kStripThreads>(p, s_win, tab_base, krow_base, colp, tid);

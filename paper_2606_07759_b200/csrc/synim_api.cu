@@ -78,13 +78,6 @@ synim_status check_device()
     return SYNIM_OK;
 }
 
-int pow2_ceil(int v)
-{
-    int p = 1;
-    while (p < v) p <<= 1;
-    return p;
-}
-
 template <typename T>
 synim_status grow(T *&ptr, size_t &have, size_t want)
 {
@@ -317,24 +310,21 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     const bool dense = (d_bbox == nullptr);
     const int ny = g->ny, nx = g->nx;
 
-    // ---- shared-memory tile sizing -------------------------------------------------------------
-    const int kPatchMax = 128, kTileMax = 96;
+    // ---- shared-memory sizing ------------------------------------------------------------------
+    // The staged box: <= 3 columns of TMA alignment slack, ring, support (or a piece of it), ring.  With a
+    // size hint the whole support is one piece; without one, and for dense modes (the support is the
+    // whole grid), 63 x 62 pieces -- by linearity a piece is its own mode and the pieces' slopes add up.
+    const int kPatchMax = 128;
     int bw = bbox_max_w, bh = bbox_max_h;
     const bool hinted = !dense && bw > 0 && bh > 0 && bw + 5 <= kPatchMax && bh + 2 <= kPatchMax;
-    int patch_pitch, patch_h;
+    int patch_pitch = 68, patch_h = 64;
     if (hinted) {
-        patch_pitch = (std::min(bw, nx) + 5 + 3) & ~3;   // <= 3 columns of TMA alignment slack, ring, support, ring
-        patch_h = std::min(bh, ny) + 2;                  // ring, support, ring
-    } else if (!dense) {
-        patch_pitch = 68;   // unknown support size: 63 x 62 pieces (larger supports are split, by linearity)
-        patch_h = 64;
-    } else {
-        patch_pitch = 96;
-        patch_h = 96;
+        patch_pitch = (std::min(bw, nx) + 5 + 3) & ~3;
+        patch_h = std::min(bh, ny) + 2;
     }
+    const int cap_w = patch_pitch - 5, cap_h = patch_h - 2;
 
     std::vector<synim::WfsDev> dev(n_wfs);
-    int tile_cap = 1;
     for (int w = 0; w < n_wfs; ++w) {
         const WfsHost &h = g->wfs[w];
         synim::WfsDev &d = dev[w];
@@ -343,67 +333,43 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         d.wmap = h.d_wmap; d.subap_row = h.d_subap_row;
         d.scale = (float)affine[w].slope_scale;
         d.M = h.M; d.n_subap = h.n_subap; d.n_pix = h.n_pix; d.row_x = h.row_x; d.row_y = h.row_y;
-        d.group = std::min(32, pow2_ceil(h.n_pix));
-        d.pad_ = 0; d.tab_off = 0; d.tab_cap = 0;
-        // tile edge when the whole support is one patch: large enough for the support's footprint
-        int tf = 64;
-        if (hinted) {
-            const double ew = (bw + 2) * std::fabs(d.inv[0]) + (bh + 2) * std::fabs(d.inv[1]);
-            const double eh = (bw + 2) * std::fabs(d.inv[3]) + (bh + 2) * std::fabs(d.inv[4]);
-            const double e = std::max(ew, eh);
-            tf = (e < 4096.0) ? (int)std::ceil(e) + 5 : kTileMax;
-        }
-        tf = std::max(8, std::min(tf, kTileMax));
-        tf = std::min(tf, h.M);
-        // tile edge when the patch is staged per tile: the source box of (t+2)^2 pixels plus 4 must fit
-        const double gx = std::fabs(d.fwd[0]) + std::fabs(d.fwd[1]), gy = std::fabs(d.fwd[3]) + std::fabs(d.fwd[4]);
-        const double lim_x = (patch_pitch - 5) / std::max(gx, 1e-12) - 1.0;
-        const double lim_y = (patch_h - 5) / std::max(gy, 1e-12) - 1.0;
-        int td = (int)std::floor(std::min({lim_x, lim_y, 64.0}));
-        td = std::max(1, std::min(td, h.M));
-        if (td >= h.n_pix) td -= td % h.n_pix;   // whole subapertures per tile when they fit
-        d.tile_fixed = tf; d.tile_dense = td;
-        tile_cap = std::max(tile_cap, std::max(tf, td));
+        d.tab_off = 0; d.tab_cap = 0;
     }
-    const int phi_h = tile_cap + 2;
-    const int phi_pitch = (tile_cap + 2) | 1;   // odd pitch: rows of a subaperture fall in different banks
-    // strip kernel: per sensor a table of (x, y) partial slopes over the window of subapertures one
-    // piece's footprint can span (the kernel derives the window from the same bounds and traps if it
-    // ever needed more)
+    // per sensor a table of (x, y) partial slopes over the window of subapertures one piece's footprint
+    // can span (the kernel derives the window from the same bounds and traps if it ever needed more)
     int tab_floats_max = 0;
-    if (!dense) {
-        const int cap_w = patch_pitch - 5, cap_h = patch_h - 2;
-        for (int w0 = 0; w0 < n_wfs; w0 += synim::kMaxWfsPerLaunch) {
-            int off = 0;
-            for (int w = w0; w < std::min(n_wfs, w0 + synim::kMaxWfsPerLaunch); ++w) {
-                synim::WfsDev &d = dev[w];
-                const double ej = (cap_w + 2) * std::fabs(d.inv[0]) + (cap_h + 2) * std::fabs(d.inv[1]);
-                const double ei = (cap_w + 2) * std::fabs(d.inv[3]) + (cap_h + 2) * std::fabs(d.inv[4]);
-                auto span = [&](double e) {   // subapertures that floor(x) .. ceil(x + e) can touch
-                    const double s_ = std::floor((std::min(e, 1.0e8) + 2.0) / d.n_pix) + 2.0;
-                    return (int)std::min<double>(s_, d.n_subap);
-                };
-                d.tab_off = off;
-                d.tab_cap = 2 * span(ej) * span(ei);
-                off += d.tab_cap;
-            }
-            tab_floats_max = std::max(tab_floats_max, (off + 3) & ~3);
+    for (int w0 = 0; w0 < n_wfs; w0 += synim::kMaxWfsPerLaunch) {
+        int off = 0;
+        for (int w = w0; w < std::min(n_wfs, w0 + synim::kMaxWfsPerLaunch); ++w) {
+            synim::WfsDev &d = dev[w];
+            const double ej = (cap_w + 2) * std::fabs(d.inv[0]) + (cap_h + 2) * std::fabs(d.inv[1]);
+            const double ei = (cap_w + 2) * std::fabs(d.inv[3]) + (cap_h + 2) * std::fabs(d.inv[4]);
+            auto span = [&](double e) {   // subapertures that floor(x) .. ceil(x + e) can touch
+                const double s_ = std::floor((std::min(e, 1.0e8) + 2.0) / d.n_pix) + 2.0;
+                return (int)std::min<double>(s_, d.n_subap);
+            };
+            d.tab_off = off;
+            d.tab_cap = 2 * span(ej) * span(ei);
+            off += d.tab_cap;
         }
+        tab_floats_max = std::max(tab_floats_max, (off + 3) & ~3);
     }
-    const size_t smem = dense ? sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)phi_pitch * phi_h)
-                              : sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)tab_floats_max) +
-                                    sizeof(int) * (size_t)(tab_floats_max / 2);
+    const size_t smem = sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)tab_floats_max) +
+                        sizeof(int) * (size_t)(tab_floats_max / 2);
     CUtensorMap tmap;
-    if (!dense) {
-        synim_status st = encode_cube_map(d_influence, n_modes, ny, nx, patch_pitch, patch_h, &tmap);
-        if (st != SYNIM_OK) return st;
-    }
+    synim_status st = encode_cube_map(d_influence, n_modes, ny, nx, patch_pitch, patch_h, &tmap);
+    if (st != SYNIM_OK) return st;
     if (smem > synim::max_dynamic_smem())
         return fail(SYNIM_ERR_CUDA, "synim_interaction_matrix: %zu bytes of shared memory exceed the device limit", smem);
 
     // ---- launches ------------------------------------------------------------------------------
+    // Dense modes: the pieces of a mode are spread over `chunks` CTAs that add into one column, so the
+    // column is cleared first (one strided memset).  Compact modes: the CTA that owns the column writes
+    // its zeros itself.
+    int chunks = 1;
     if (dense) {
-        // several CTAs accumulate into one column: clear the rows first (one strided memset)
+        const int npieces = ((nx - 1 + cap_w) / cap_w) * ((ny - 1 + cap_h) / cap_h);
+        chunks = std::max(1, std::min(npieces, 8));
         if (ld == g->rows) SYNIM_CUDA(cudaMemsetAsync(d_out, 0, sizeof(float) * (size_t)g->rows * n_modes, s));
         else SYNIM_CUDA(cudaMemset2DAsync(d_out, sizeof(float) * (size_t)ld, 0, sizeof(float) * (size_t)g->rows, n_modes, s));
     }
@@ -415,22 +381,18 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
         p.addr_bias = 0x4B400000u << 2;
         p.patch_pitchf = (float)patch_pitch;
-        p.patch_pitch = patch_pitch; p.patch_h = patch_h; p.phi_pitch = phi_pitch; p.phi_h = phi_h;
+        p.patch_pitch = patch_pitch; p.patch_h = patch_h;
         for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
         p.tab_floats = nw > 0 ? (dev[w0 + nw - 1].tab_off + dev[w0 + nw - 1].tab_cap + 3) & ~3 : 0;
+        p.chunks = chunks;
         if (dense) {
             p.zero_begin = 0; p.zero_count = 0;
-            p.chunks = 8;
-            p.jobs_per_mode = nw * p.chunks;
         } else {
             p.zero_begin = g->wfs[w0].row_x;
             const WfsHost &last = g->wfs[w0 + nw - 1];
             p.zero_count = last.row_x + 2 * last.n_valid - p.zero_begin;
-            p.chunks = 1;
-            p.jobs_per_mode = 1;
         }
-        if (dense) SYNIM_CUDA(synim::launch_interaction_matrix(p, smem, s));
-        else SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));
+        SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));
     }
     return SYNIM_OK;
 }

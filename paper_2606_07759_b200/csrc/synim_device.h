@@ -1,5 +1,5 @@
 // synim_device.h -- structures shared by the host side of the C ABI (synim_api.cu) and the
-// sm_100a kernels (synim_kernels.cu).  Internal; the public interface is include/synim.h.
+// sm_100a kernels (synim_strip.cu, synim_kernels.cu).  Internal; the public interface is include/synim.h.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -7,8 +7,7 @@
 namespace synim {
 
 constexpr int kMaxWfsPerLaunch = 16;   // per-launch WFS batch (kernel-parameter space is 4 KB)
-constexpr int kThreads = 256;          // CTA size of the interaction-matrix kernel
-constexpr int kWmapPadRows = 8;        // rows of zeros below each sensor's weight map (strip kernel look-ahead)
+constexpr int kWmapPadRows = 8;        // rows of zeros below each sensor's weight map (the kernel's look-ahead)
 
 // One sensor as the kernel sees it.  All coordinates are ABSOLUTE pixel indices: WFS pixel (i, j)
 // (row, column) samples the source grid at
@@ -24,11 +23,7 @@ struct WfsDev {
     float scale;             // slope_scale
     int M, n_subap, n_pix;
     int row_x, row_y;        // first row of the x / y slopes of this sensor inside a column
-    int tile_fixed;          // max edge (WFS pixels) of a D tile when the whole support is one patch
-    int tile_dense;          // max edge when the patch is re-staged per tile (its source box must fit)
-    int group;               // lanes that share one subaperture in the reduction (power of 2 <= 32)
-    int tab_off, tab_cap;    // strip kernel: this sensor's slice of the CTA's slope table (floats)
-    int pad_;
+    int tab_off, tab_cap;    // this sensor's slice of the CTA's slope table (floats)
 };
 
 struct ImParams {
@@ -38,21 +33,18 @@ struct ImParams {
     float *out;              // column-major IM
     long long ld;
     int n_modes, ny, nx, n_wfs;
-    int patch_pitch, patch_h;   // shared-memory patch capacity, floats x rows
-    int phi_pitch, phi_h;       // shared-memory phi tile capacity including the 1-pixel halo
-    int zero_begin, zero_count; // rows [zero_begin, zero_begin+zero_count) of every column are zero-filled
-                                // by the mode's CTA before it accumulates (0: caller pre-zeroed)
-    int jobs_per_mode;          // 1: one CTA per mode walks every sensor; else n_wfs*chunks CTAs per mode
-    int chunks;                 // tile chunks per sensor when jobs_per_mode > 1
-    float patch_pitchf;         // strip kernel: patch_pitch as float (an FFMA operand straight from constant memory)
-    unsigned addr_bias;         // strip kernel: (bits of 1.5*2^23) << 2 mod 2^32, see process_strip
-    int tab_floats;             // strip kernel: size of the CTA's slope table (multiple of 4)
+    int patch_pitch, patch_h;   // the staged box (TMA), floats x rows
+    int zero_begin, zero_count; // rows [zero_begin, zero_begin+zero_count) of a column are zeroed by the mode's
+                                // CTA (0: the caller cleared them, dense modes)
+    int chunks;                 // CTAs per mode (grid.y): the pieces of a dense mode are spread over them
+    float patch_pitchf;         // patch_pitch as float (an FFMA operand straight from constant memory)
+    unsigned addr_bias;         // (bits of 1.5*2^23) << 2 mod 2^32, see process_strip
+    int tab_floats;             // size of the CTA's slope table (multiple of 4)
     WfsDev wfs[kMaxWfsPerLaunch];
 };
 
-// launchers (synim_kernels.cu); all asynchronous on `stream`, return the launch status
-cudaError_t launch_interaction_matrix(const ImParams &p, size_t smem_bytes, cudaStream_t stream);
-// compact-support path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
+// launchers; all asynchronous on `stream`, return the launch status.
+// The hot path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
 // {patch_pitch, patch_h, 1}
 cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,

@@ -378,7 +378,8 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     // [ TMA box: patch_pitch x patch_h floats | table: tab_floats | rows: tab_floats / 2 ints ]
     extern __shared__ __align__(128) float patch[];
     __shared__ __align__(8) uint64_t bar;
-    __shared__ int4 s_win[kMaxWfsPerLaunch];
+    __shared__ int4 s_win[kMaxWfsPerLaunch];   // window of subapertures of each sensor: a0, b0, na, nb
+    __shared__ int4 s_box[kMaxWfsPerLaunch];   // footprint of each sensor: i0, i1, j0, j1
     __shared__ int s_next;   // next strip of the current piece
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int mode = blockIdx.x;
@@ -387,7 +388,10 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     const uint32_t tab_base = raw_base + (uint32_t)(p.patch_pitch * p.patch_h) * 4u;
     const uint32_t krow_base = tab_base + (uint32_t)p.tab_floats * 4u;   // IM row of each (a, b) of the windows
 
-    const int4 b = __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode);
+    // dense modes (no bboxes): the support is the whole grid, split into pieces; blockIdx.y takes every
+    // gridDim.y-th piece, and the pieces' slopes add up in the column, which the host has cleared
+    const int chunk = blockIdx.y, nchunk = gridDim.y;
+    const int4 b = p.bbox != nullptr ? __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode) : make_int4(0, 0, p.nx - 1, p.ny - 1);
     const int bx0 = max(b.x, 0), by0 = max(b.y, 0), bx1 = min(b.z, p.nx - 1), by1 = min(b.w, p.ny - 1);
     const bool empty = bx1 < bx0 || by1 < by0;
     // diagonal extents of the support: min/max of x+y and of x-y over its non-zero pixels (the bbox's own
@@ -404,15 +408,16 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     const int cap_w = p.patch_pitch - 5, cap_h = p.patch_h - 2;
     const int npcx = empty ? 0 : (bx1 - bx0 + cap_w) / cap_w, npcy = empty ? 0 : (by1 - by0 + cap_h) / cap_h;
     const int npieces = npcx * npcy;
-    const bool multi = npieces > 1;
+    const bool multi = npieces > 1 || nchunk > 1;
     const uint32_t box_bytes = (uint32_t)(p.patch_pitch * p.patch_h) * 4u;
 
-    if (tid == 0 && npieces > 0) {
+    if (tid == 0 && chunk < npieces) {
         mbar_init(&bar, 1);
         fence_barrier_init();
         fence_proxy_async();
         mbar_expect_tx(&bar, box_bytes);
-        tma_load_box(patch, &tmap, &bar, (bx0 - 1) & ~3, by0 - 1, mode);
+        const int fy = chunk / npcx, fx = chunk - fy * npcx;
+        tma_load_box(patch, &tmap, &bar, (bx0 + fx * cap_w - 1) & ~3, by0 + fy * cap_h - 1, mode);
     }
     for (int e = tid; e < p.tab_floats; e += kStripThreads) sts_f32(tab_base + (uint32_t)e * 4u, 0.0f);
     if (tid < kMaxWfsPerLaunch) s_win[tid] = make_int4(0, 0, 0, 0);
@@ -435,7 +440,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     }
     {
         uint32_t parity = 0;
-        for (int pc = 0; pc < npieces; ++pc) {
+        for (int pc = chunk; pc < npieces; pc += nchunk) {
             const int pcy = pc / npcx, pcx = pc - pcy * npcx;
             const int qx0 = bx0 + pcx * cap_w, qx1 = min(qx0 + cap_w - 1, bx1);
             const int qy0 = by0 + pcy * cap_h, qy1 = min(qy0 + cap_h - 1, by1);
@@ -448,24 +453,12 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             cb.pitchf = p.patch_pitchf;
             cb.s_lo = (float)(sg0 - 2 - (cb.x0 + cb.y0)) - 0.01f; cb.s_hi = (float)(sg1 + 2 - (cb.x0 + cb.y0)) + 0.01f;
             cb.d_lo = (float)(dg0 - 2 - (cb.x0 - cb.y0)) - 0.01f; cb.d_hi = (float)(dg1 + 2 - (cb.x0 - cb.y0)) + 0.01f;
-            mbar_wait(&bar, parity);
-            parity ^= 1u;
-
-            // By linearity a piece is its own mode, zero outside its box: when the support was split, whatever
-            // the box holds on the piece's ring is read as 0.
-            if (multi) {   // clear the ring just staged (pixels cw and ch are the far ring)
-                const uint32_t org = raw_base + (uint32_t)slack * 4u, rp4 = (uint32_t)p.patch_pitch * 4u;
-                for (int e = tid; e <= cb.cw; e += kComputeThreads) { sts_f32(org + (uint32_t)e * 4u, 0.0f); sts_f32(org + (uint32_t)cb.ch * rp4 + (uint32_t)e * 4u, 0.0f); }
-                for (int e = tid; e <= cb.ch; e += kComputeThreads) { sts_f32(org + (uint32_t)e * rp4, 0.0f); sts_f32(org + (uint32_t)e * rp4 + (uint32_t)cb.cw * 4u, 0.0f); }
-                bar_sync(1, kComputeThreads);
-            }
-
             // lane w: footprint of this piece on sensor w.  phi(i,j) can be non-zero only strictly inside the
             // image, under the inverse map, of the piece's open octagon: the box (qx0-1,qx1+1)x(qy0-1,qy1+1)
             // cut by sg0-2 < x+y < sg1+2 and dg0-2 < x-y < dg1+2.  So D(i,j) only for floor(jmin) <= j <=
             // ceil(jmax) (one pixel of stencil either side), clipped to the sensor.
-            int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_na = 0, r_nb = 0;
-            if (lane < p.n_wfs) {
+            if (warp == 0 && lane < p.n_wfs) {   // once per CTA, while the box is still in flight
+                int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_a0 = 0, r_b0 = 0, r_na = 0, r_nb = 0;
                 const WfsDev &W = p.wfs[lane];
                 const double X0 = qx0 - 1, X1 = qx1 + 1, Y0 = qy0 - 1, Y1 = qy1 + 1;
                 const double S0 = sg0 - 2, S1 = sg1 + 2, D0 = dg0 - 2, D1 = dg1 + 2;
@@ -490,25 +483,45 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                 r_i0 = max(0, (int)floor(fmax(imin, -lim))); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)));
                 int4 win = make_int4(0, 0, 0, 0);
                 if (r_j1 >= r_j0 && r_i1 >= r_i0) {
-                    r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
                     r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
                     r_nb = r_j1 / W.n_pix - r_b0 + 1;
                     r_na = r_i1 / W.n_pix - r_a0 + 1;
                     win = make_int4(r_a0, r_b0, r_na, r_nb);
                     if (win.z * win.w * 2 > W.tab_cap) __trap();   // the host sized the table from the same bounds
                 }
-                if (warp == 0) s_win[lane] = win;   // read by scatter_table after a barrier
+                s_box[lane] = make_int4(r_i0, r_i1, r_j0, r_j1);
+                s_win[lane] = win;   // also read by scatter_table
+            }
+            mbar_wait(&bar, parity);
+            parity ^= 1u;
+
+            // By linearity a piece is its own mode, zero outside its box: when the support was split, whatever
+            // the box holds on the piece's ring is read as 0.
+            if (multi) {   // clear the ring just staged (pixels cw and ch are the far ring)
+                const uint32_t org = raw_base + (uint32_t)slack * 4u, rp4 = (uint32_t)p.patch_pitch * 4u;
+                for (int e = tid; e <= cb.cw; e += kComputeThreads) { sts_f32(org + (uint32_t)e * 4u, 0.0f); sts_f32(org + (uint32_t)cb.ch * rp4 + (uint32_t)e * 4u, 0.0f); }
+                for (int e = tid; e <= cb.ch; e += kComputeThreads) { sts_f32(org + (uint32_t)e * rp4, 0.0f); sts_f32(org + (uint32_t)e * rp4 + (uint32_t)cb.cw * 4u, 0.0f); }
+            }
+            bar_sync(1, kComputeThreads);   // footprints (and a cleared ring) visible
+
+            int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_nb = 0;
+            if (lane < p.n_wfs) {
+                const int4 fb = s_box[lane], fw = s_win[lane];
+                r_i0 = fb.x; r_i1 = fb.y; r_j0 = fb.z; r_j1 = fb.w;
+                r_a0 = fw.x; r_b0 = fw.y; r_nb = fw.w;
+                if (r_j1 >= r_j0 && r_i1 >= r_i0) r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
             }
             // the IM rows of the windows' subapertures, needed only when the table is stored: fetched now,
             // asynchronously, so that the store at the end waits for nothing (sensor w by warp w mod 4)
             for (int w = warp; w < p.n_wfs; w += kComputeWarps) {
-                const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
-                const int na = __shfl_sync(kFull, r_na, w);
+                const int4 fw = s_win[w];   // a0, b0, na, nb
                 const WfsDev &W = p.wfs[w];
-                for (int a = 0; a < na; ++a)
-                    for (int bq = lane; bq < nb; bq += 32)
-                        cp_async_4(krow_base + (uint32_t)((W.tab_off >> 1) + a * nb + bq) * 4u,
-                                   W.subap_row + (a0 + a) * W.n_subap + (b0 + bq));
+                const int n = fw.z * fw.w;
+                const unsigned magic = 0xFFFFFFFFu / (unsigned)max(fw.w, 1) + 1u;   // (wraps to 0 for 1)
+                for (int e = lane; e < n; e += 32) {
+                    const int ra = fw.w == 1 ? e : (int)__umulhi((unsigned)e, magic), rb = e - ra * fw.w;
+                    cp_async_4(krow_base + (uint32_t)((W.tab_off >> 1) + e) * 4u, W.subap_row + (fw.x + ra) * W.n_subap + (fw.y + rb));
+                }
             }
             int incl = r_n;
 #pragma unroll
@@ -536,8 +549,8 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             if (multi) {
                 cp_async_wait_all();
                 bar_sync(1, kComputeThreads);   // every warp is done with this box and this piece's table
-                if (pc + 1 < npieces && tid == 0) {   // the box was being sampled until now
-                    const int ny_ = (pc + 1) / npcx, nx_ = (pc + 1) - ny_ * npcx;
+                if (pc + nchunk < npieces && tid == 0) {   // the box was being sampled until now
+                    const int ny_ = (pc + nchunk) / npcx, nx_ = (pc + nchunk) - ny_ * npcx;
                     fence_proxy_async();
                     mbar_expect_tx(&bar, box_bytes);
                     tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
@@ -563,7 +576,7 @@ cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_
     if (e != cudaSuccess) return e;
     CUtensorMap tm;
     memcpy(&tm, tensor_map, sizeof(tm));
-    synim_strip_kernel<<<(unsigned)p.n_modes, kStripThreads, smem_bytes, stream>>>(p, tm);
+    synim_strip_kernel<<<dim3((unsigned)p.n_modes, (unsigned)(p.chunks > 0 ? p.chunks : 1)), kStripThreads, smem_bytes, stream>>>(p, tm);
     return cudaGetLastError();
 }
 

@@ -33,7 +33,10 @@ namespace synim {
 
 namespace {
 
-constexpr int kComputeWarps = 4, kComputeThreads = 32 * kComputeWarps;
+#ifndef SYNIM_STRIP_WARPS
+#define SYNIM_STRIP_WARPS 4
+#endif
+constexpr int kComputeWarps = SYNIM_STRIP_WARPS, kComputeThreads = 32 * kComputeWarps;
 constexpr int kStripThreads = kComputeThreads;
 #ifndef SYNIM_STRIP_MINB
 #define SYNIM_STRIP_MINB 7
@@ -217,8 +220,6 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     const int segL = __shfl_up_sync(kFull, seg, 1);
     const bool head = isD && (lane == 1 || segL != seg);
     unsigned okm = 0;
-    int nsteps = 0;
-    while ((1 << nsteps) < min(npx, kStripCols)) ++nsteps;
 #pragma unroll
     for (int s = 0; s < 5; ++s) {
         const int sd = __shfl_down_sync(kFull, seg, 1 << s);
@@ -241,11 +242,9 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         unsigned m = okm;
         asm volatile("" : "+r"(m));   // keeps the five lane masks out of predicate registers between flushes
 #pragma unroll
-        for (int s = 0; s < 5; ++s) {
-            if (s < nsteps) {   // warp-uniform
-                const float tx = __shfl_down_sync(kFull, sx, 1 << s), ty = __shfl_down_sync(kFull, sy, 1 << s);
-                if ((m >> s) & 1u) { sx += tx; sy += ty; }
-            }
+        for (int s = 0; s < 5; ++s) {   // (a step beyond the segment length has no lane mask set: cheaper than a branch)
+            const float tx = __shfl_down_sync(kFull, sx, 1 << s), ty = __shfl_down_sync(kFull, sy, 1 << s);
+            if ((m >> s) & 1u) { sx += tx; sy += ty; }
         }
         if (head && (sx != 0.0f || sy != 0.0f) && a_cur < S.n_subap) {
             red_shared_f32(tent, sx);   // another warp may hold the other columns of this subaperture
@@ -304,7 +303,8 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     float sx = 0.0f, sy = 0.0f;
 #pragma unroll 1
     for (int d = d_lo; d <= d_hi; d += kRows) {
-        zp.step();
+#pragma unroll
+        for (int q = 0; q < (kComputeWarps >= 4 ? 1 : 4 / kComputeWarps); ++q) zp.step();
         // weights of the next kRows rows, one iteration ahead of their use
         woff += wstride;
         float wnx[kRows];

@@ -33,6 +33,9 @@ namespace synim {
 
 namespace {
 
+#ifndef SYNIM_STRIP_UNROLL
+#define SYNIM_STRIP_UNROLL 1
+#endif
 #ifndef SYNIM_STRIP_WARPS
 #define SYNIM_STRIP_WARPS 4
 #endif
@@ -44,6 +47,7 @@ constexpr int kStripThreads = kComputeThreads;
 #ifndef SYNIM_STRIP_ROWS
 #define SYNIM_STRIP_ROWS 2
 #endif
+constexpr int kStripUnroll = SYNIM_STRIP_UNROLL;
 constexpr int kStripRows = SYNIM_STRIP_ROWS;                // pixel rows per loop iteration (independent samples in flight per lane)
 static_assert(2 * kStripRows <= kWmapPadRows, "weight look-ahead runs past the rows of zeros");
 constexpr int kStripCols = 30;               // D columns per strip: lanes 1..30, halo on lanes 0 and 31
@@ -301,7 +305,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
 #pragma unroll
     for (int k = 0; k < kRows; ++k) wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
     float sx = 0.0f, sy = 0.0f;
-#pragma unroll 1
+#pragma unroll(kStripUnroll)
     for (int d = d_lo; d <= d_hi; d += kRows) {
 #pragma unroll
         for (int q = 0; q < (kComputeWarps >= 4 ? 1 : 4 / kComputeWarps); ++q) zp.step();

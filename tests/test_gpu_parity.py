@@ -132,6 +132,57 @@ def test_config5_dense_zernike_modes(S):
     assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
 
 
+def _full_size_sampled(S, cfg, n_sample, seed):
+    """The whole config in bench.py's launch configuration (device-computed supports, size hint);
+    sampled columns against the oracle, the rest through properties that hold at any size."""
+    import copy
+    import torch
+    wl = W.make_config(cfg)
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    cube = torch.from_numpy(wl.cube).cuda()
+    bbox = diag = None
+    bmax = (0, 0)
+    if wl.bbox is not None:
+        bbox, diag = S.compute_supports(cube)
+        assert np.array_equal(bbox.cpu().numpy(), wl.bbox)
+        bmax = S.bbox_extent(bbox)
+    out = torch.full((wl.n_modes, geom.num_rows), float("nan"), dtype=torch.float32, device="cuda")
+    S.interaction_matrix(geom, cube, bbox, S.affines_of(wl), [w.slope_scale for w in wl.wfs], out=out, bbox_max=bmax,
+                         diag=diag)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(out).all())          # every element of every column was written
+    sel = np.sort(np.random.default_rng(seed).choice(wl.n_modes, size=n_sample, replace=False))
+    got = out[torch.from_numpy(sel).cuda()].cpu().numpy().T.copy()
+    sub = copy.copy(wl)
+    sub.cube = wl.cube[sel]
+    sub.bbox = None if wl.bbox is None else wl.bbox[sel]
+    assert_parity(got, O.interaction_matrix(wl, modes=sel), sub)
+    if wl.bbox is not None:
+        # compact support: a column has at most (footprint / subaperture + 2)^2 non-zero slopes per sensor
+        nnz = (out != 0).sum(dim=1).cpu().numpy()
+        r0, bound = 0, 0
+        for w in wl.wfs:
+            aff = np.asarray(S.compose_affine(w.phys))[:6].reshape(2, 3)[:, :2]
+            ext = (max(bmax) + 2) * np.abs(np.linalg.inv(aff)).sum(axis=1).max() + 2
+            bound += 2 * (int(ext // w.n_pix) + 2) ** 2
+        assert nnz.max() <= bound, (int(nnz.max()), bound)
+        assert nnz.min() >= 0 and (nnz > 0).mean() > 0.9     # nearly every actuator is seen by some sensor
+    geom.destroy()
+
+
+def test_config3_full_size_in_the_bench_configuration(S):
+    _full_size_sampled(S, 3, 12, 11)
+
+
+def test_config2_and_config4_full_size(S):
+    _full_size_sampled(S, 2, 16, 12)
+    _full_size_sampled(S, 4, 8, 14)
+
+
+def test_config5_full_size_dense(S):
+    _full_size_sampled(S, 5, 3, 15)
+
+
 def test_dense_path_on_zonal_cube_equals_bbox_path(S):
     """bbox = NULL must give the same matrix as the tile-skipping path (skipping is exact, R15)."""
     wl = W.make_config(1, max_modes=24)

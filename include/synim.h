@@ -147,10 +147,14 @@ synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int
 synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *max_w, int32_t *max_h,
                                void *stream);
 
-/* Convenience wrapper with HOST buffers, for one-shot use and end-to-end timing: copies the cube
- * (and bboxes, if given) to the device, runs synim_interaction_matrix, copies the IM back and
- * synchronises.  h_out is column-major with ld = synim_num_rows().  Pinned host memory makes the
- * copies asynchronous but is not required. */
+/* Convenience wrapper with HOST buffers, for one-shot use and end-to-end timing: brings the cube to
+ * the device, runs synim_interaction_matrix, copies the IM back and synchronises.  h_out is column-major
+ * with ld = synim_num_rows().  With h_bbox (HOST int32 [n_modes][4], every bbox inside the grid, else
+ * INVALID_ARG) only the supports cross the bus: each mode's bbox plus the ring of zeros the kernel stages
+ * with it is packed into a pinned buffer of [n_modes][max_h + 2][roundup4(max_w + 5)] floats (host
+ * threads), copied, and the kernel reads the packed cube through per-mode origins.  With h_bbox == NULL
+ * (dense modes) the whole cube is copied.  Pinned h_influence / h_out make the copies asynchronous but
+ * are not required. */
 synim_status synim_interaction_matrix_host(const synim_geometry *geom, const float *h_influence, int32_t n_modes,
                                            const int32_t *h_bbox, const synim_wfs_affine *affine,
                                            synim_slope_mode mode, float *h_out, void *stream);

@@ -14,6 +14,7 @@
 #include <cstdlib>
 #include <mutex>
 #include <new>
+#include <thread>
 #include <vector>
 
 namespace {
@@ -60,8 +61,10 @@ struct synim_geometry {
     mutable size_t ws_cube_bytes = 0;
     mutable float *ws_out = nullptr;
     mutable size_t ws_out_bytes = 0;
-    mutable int *ws_bbox = nullptr;
+    mutable int *ws_bbox = nullptr;      // bboxes [n][4], then origins [n][2]
     mutable size_t ws_bbox_bytes = 0;
+    mutable float *h_stage = nullptr;    // pinned: the packed supports on their way to the device
+    mutable size_t h_stage_bytes = 0;
 };
 
 namespace {
@@ -191,6 +194,7 @@ void synim_destroy(synim_geometry *g)
     if (g->ws_cube) cudaFree(g->ws_cube);
     if (g->ws_out) cudaFree(g->ws_out);
     if (g->ws_bbox) cudaFree(g->ws_bbox);
+    if (g->h_stage) cudaFreeHost(g->h_stage);
     delete g;
 }
 
@@ -287,10 +291,14 @@ int64_t synim_row_offset(const synim_geometry *g, int32_t w)
     return (g && w >= 0 && w < (int)g->wfs.size()) ? g->wfs[w].row_x : -1;
 }
 
-synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_influence, int32_t n_modes,
-                                      const int32_t *d_bbox, const int32_t *d_diag, int32_t bbox_max_w, int32_t bbox_max_h,
-                                      const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out, int64_t ld,
-                                      void *stream)
+// The launch behind both entry points.  The cube may be PACKED (synim_interaction_matrix_host): mode m
+// then holds only the neighbourhood of its support, cube_ny x cube_nx pixels whose pixel (0, 0) is source
+// pixel d_origin[m] = (ox, oy); bboxes and affine maps stay in source-grid coordinates.
+static synim_status run_interaction_matrix(const synim_geometry *g, const float *d_influence, int cube_ny, int cube_nx,
+                                           const int32_t *d_origin, int32_t n_modes, const int32_t *d_bbox,
+                                           const int32_t *d_diag, int32_t bbox_max_w, int32_t bbox_max_h,
+                                           const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out, int64_t ld,
+                                           void *stream)
 {
     if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
     if (mode == SYNIM_SLOPES_GTILT)
@@ -357,7 +365,7 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     const size_t smem = sizeof(float) * ((size_t)patch_pitch * patch_h + (size_t)tab_floats_max) +
                         sizeof(int) * (size_t)(tab_floats_max / 2);
     CUtensorMap tmap;
-    synim_status st = encode_cube_map(d_influence, n_modes, ny, nx, patch_pitch, patch_h, &tmap);
+    synim_status st = encode_cube_map(d_influence, n_modes, cube_ny, cube_nx, patch_pitch, patch_h, &tmap);
     if (st != SYNIM_OK) return st;
     if (smem > synim::max_dynamic_smem())
         return fail(SYNIM_ERR_CUDA, "synim_interaction_matrix: %zu bytes of shared memory exceed the device limit", smem);
@@ -377,7 +385,7 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         const int nw = std::min(synim::kMaxWfsPerLaunch, n_wfs - w0);
         synim::ImParams p;
         std::memset(&p, 0, sizeof(p));
-        p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.out = d_out; p.ld = ld;
+        p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.origin = d_origin; p.out = d_out; p.ld = ld;
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
         p.addr_bias = 0x4B400000u << 2;
         p.patch_pitchf = (float)patch_pitch;
@@ -395,6 +403,16 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
         SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));
     }
     return SYNIM_OK;
+}
+
+synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_influence, int32_t n_modes,
+                                      const int32_t *d_bbox, const int32_t *d_diag, int32_t bbox_max_w, int32_t bbox_max_h,
+                                      const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out, int64_t ld,
+                                      void *stream)
+{
+    if (!g) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
+    return run_interaction_matrix(g, d_influence, g->ny, g->nx, nullptr, n_modes, d_bbox, d_diag, bbox_max_w, bbox_max_h, affine,
+                                  mode, d_out, ld, stream);
 }
 
 synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx, int32_t *d_bbox,
@@ -438,24 +456,76 @@ synim_status synim_interaction_matrix_host(const synim_geometry *g, const float 
     if (!h_influence || !h_out) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_host: NULL host buffer");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     std::lock_guard<std::mutex> guard(g->lock);
-    const size_t cube_bytes = sizeof(float) * (size_t)n_modes * g->ny * g->nx;
+    const int ny = g->ny, nx = g->nx;
     const size_t out_bytes = sizeof(float) * (size_t)n_modes * (size_t)g->rows;
-    const size_t bbox_bytes = h_bbox ? sizeof(int) * 4 * (size_t)n_modes : 0;
     synim_status st;
-    if ((st = grow(g->ws_cube, g->ws_cube_bytes, cube_bytes)) != SYNIM_OK) return st;
     if ((st = grow(g->ws_out, g->ws_out_bytes, std::max<size_t>(out_bytes, 16))) != SYNIM_OK) return st;
-    if (h_bbox && (st = grow(g->ws_bbox, g->ws_bbox_bytes, bbox_bytes)) != SYNIM_OK) return st;
-    int bw = 0, bh = 0;
-    if (h_bbox) {
+
+    if (!h_bbox) {   // dense modes: the whole cube crosses the bus
+        const size_t cube_bytes = sizeof(float) * (size_t)n_modes * ny * nx;
+        if ((st = grow(g->ws_cube, g->ws_cube_bytes, cube_bytes)) != SYNIM_OK) return st;
+        SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, h_influence, cube_bytes, cudaMemcpyHostToDevice, s));
+        st = run_interaction_matrix(g, g->ws_cube, ny, nx, nullptr, n_modes, nullptr, nullptr, 0, 0, affine, mode, g->ws_out,
+                                    g->rows, s);
+    } else {
+        // Compact supports: only each mode's bbox (plus the ring of zeros the kernel stages with it) crosses
+        // the bus -- 29 MB instead of 4.67 GB at config 3.  Mode m is packed into a pny x pnx image whose
+        // pixel (0, 0) is source pixel (ox, oy) = ((x0-1) & ~3, y0-1): exactly the origin of the box the
+        // kernel's TMA load asks for, 16-byte aligned like it.
+        int bw = 0, bh = 0;
         for (int m = 0; m < n_modes; ++m) {
-            bw = std::max(bw, h_bbox[4 * m + 2] - h_bbox[4 * m] + 1);
-            bh = std::max(bh, h_bbox[4 * m + 3] - h_bbox[4 * m + 1] + 1);
+            const int32_t *b = h_bbox + 4 * (size_t)m;
+            if (b[2] < b[0] || b[3] < b[1]) continue;
+            if (b[0] < 0 || b[1] < 0 || b[2] >= nx || b[3] >= ny)
+                return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_host: bbox of mode %d leaves the grid", m);
+            bw = std::max(bw, b[2] - b[0] + 1);
+            bh = std::max(bh, b[3] - b[1] + 1);
         }
-        SYNIM_CUDA(cudaMemcpyAsync(g->ws_bbox, h_bbox, bbox_bytes, cudaMemcpyHostToDevice, s));
+        const int pnx = std::max(8, (bw + 5 + 3) & ~3), pny = std::max(4, bh + 2);
+        const size_t img = (size_t)pnx * pny, cube_bytes = sizeof(float) * img * n_modes;
+        const size_t meta_bytes = sizeof(int) * 6 * (size_t)n_modes;   // bboxes [n][4], origins [n][2]
+        if ((st = grow(g->ws_cube, g->ws_cube_bytes, cube_bytes)) != SYNIM_OK) return st;
+        if ((st = grow(g->ws_bbox, g->ws_bbox_bytes, meta_bytes)) != SYNIM_OK) return st;
+        if (g->h_stage_bytes < cube_bytes + meta_bytes) {
+            if (g->h_stage) cudaFreeHost(g->h_stage);
+            g->h_stage = nullptr; g->h_stage_bytes = 0;
+            cudaError_t e = cudaMallocHost(reinterpret_cast<void **>(&g->h_stage), cube_bytes + meta_bytes);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaMallocHost(staging)");
+            g->h_stage_bytes = cube_bytes + meta_bytes;
+        }
+        float *stage = g->h_stage;
+        int *meta = reinterpret_cast<int *>(reinterpret_cast<char *>(g->h_stage) + cube_bytes);
+        std::memcpy(meta, h_bbox, sizeof(int) * 4 * (size_t)n_modes);
+        int *origin = meta + 4 * (size_t)n_modes;
+        auto pack = [&](int m0, int m1) {
+            for (int m = m0; m < m1; ++m) {
+                const int32_t *b = h_bbox + 4 * (size_t)m;
+                float *dst = stage + img * m;
+                std::memset(dst, 0, sizeof(float) * img);
+                origin[2 * m] = 0; origin[2 * m + 1] = 0;
+                if (b[2] < b[0] || b[3] < b[1]) continue;
+                const int ox = (b[0] - 1) & ~3, oy = b[1] - 1;
+                origin[2 * m] = ox; origin[2 * m + 1] = oy;
+                const float *src = h_influence + (size_t)m * ny * nx;
+                const size_t row_bytes = sizeof(float) * (size_t)(b[2] - b[0] + 1);
+                for (int y = b[1]; y <= b[3]; ++y)
+                    std::memcpy(dst + (size_t)(y - oy) * pnx + (b[0] - ox), src + (size_t)y * nx + b[0], row_bytes);
+            }
+        };
+        const int nthreads = (int)std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
+        if (nthreads == 1 || n_modes < 64) {
+            pack(0, n_modes);
+        } else {
+            std::vector<std::thread> pool;
+            for (int t = 0; t < nthreads; ++t)
+                pool.emplace_back(pack, (int)((long long)n_modes * t / nthreads), (int)((long long)n_modes * (t + 1) / nthreads));
+            for (auto &th : pool) th.join();
+        }
+        SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, stage, cube_bytes, cudaMemcpyHostToDevice, s));
+        SYNIM_CUDA(cudaMemcpyAsync(g->ws_bbox, meta, meta_bytes, cudaMemcpyHostToDevice, s));
+        st = run_interaction_matrix(g, g->ws_cube, pny, pnx, g->ws_bbox + 4 * (size_t)n_modes, n_modes, g->ws_bbox, nullptr, bw, bh,
+                                    affine, mode, g->ws_out, g->rows, s);
     }
-    SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, h_influence, cube_bytes, cudaMemcpyHostToDevice, s));
-    st = synim_interaction_matrix(g, g->ws_cube, n_modes, h_bbox ? g->ws_bbox : nullptr, nullptr, bw, bh, affine, mode, g->ws_out,
-                                  g->rows, s);
     if (st != SYNIM_OK) return st;
     SYNIM_CUDA(cudaMemcpyAsync(h_out, g->ws_out, out_bytes, cudaMemcpyDeviceToHost, s));
     SYNIM_CUDA(cudaStreamSynchronize(s));

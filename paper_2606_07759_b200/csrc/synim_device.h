@@ -30,6 +30,7 @@ struct ImParams {
     const float *cube;       // [n_modes][ny][nx]
     const int *bbox;         // [n_modes][4] or nullptr
     const int *diag;         // [n_modes][4] min/max of x+y, min/max of x-y over the support, or nullptr
+    const int *origin;       // [n_modes][2] source pixel of cube pixel (0, 0) of each mode (packed cube), or nullptr
     float *out;              // column-major IM
     long long ld;
     int n_modes, ny, nx, n_wfs;

@@ -398,6 +398,8 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     const int4 b = p.bbox != nullptr ? __ldg(reinterpret_cast<const int4 *>(p.bbox) + mode) : make_int4(0, 0, p.nx - 1, p.ny - 1);
     const int bx0 = max(b.x, 0), by0 = max(b.y, 0), bx1 = min(b.z, p.nx - 1), by1 = min(b.w, p.ny - 1);
     const bool empty = bx1 < bx0 || by1 < by0;
+    // a packed cube holds mode m from source pixel org on (org.x is a multiple of 4: the alignment carries over)
+    const int2 org = p.origin != nullptr ? __ldg(reinterpret_cast<const int2 *>(p.origin) + mode) : make_int2(0, 0);
     // diagonal extents of the support: min/max of x+y and of x-y over its non-zero pixels (the bbox's own
     // when the caller has none)
     int sg0 = b.x + b.y, sg1 = b.z + b.w, dg0 = b.x - b.w, dg1 = b.z - b.y;
@@ -421,7 +423,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
         fence_proxy_async();
         mbar_expect_tx(&bar, box_bytes);
         const int fy = chunk / npcx, fx = chunk - fy * npcx;
-        tma_load_box(patch, &tmap, &bar, (bx0 + fx * cap_w - 1) & ~3, by0 + fy * cap_h - 1, mode);
+        tma_load_box(patch, &tmap, &bar, ((bx0 + fx * cap_w - 1) & ~3) - org.x, by0 + fy * cap_h - 1 - org.y, mode);
     }
     for (int e = tid; e < p.tab_floats; e += kStripThreads) sts_f32(tab_base + (uint32_t)e * 4u, 0.0f);
     if (tid < kMaxWfsPerLaunch) s_win[tid] = make_int4(0, 0, 0, 0);
@@ -557,7 +559,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                     const int ny_ = (pc + nchunk) / npcx, nx_ = (pc + nchunk) - ny_ * npcx;
                     fence_proxy_async();
                     mbar_expect_tx(&bar, box_bytes);
-                    tma_load_box(patch, &tmap, &bar, (bx0 + nx_ * cap_w - 1) & ~3, by0 + ny_ * cap_h - 1, mode);
+                    tma_load_box(patch, &tmap, &bar, ((bx0 + nx_ * cap_w - 1) & ~3) - org.x, by0 + ny_ * cap_h - 1 - org.y, mode);
                 }
                 scatter_table<true, kComputeThreads>(p, s_win, tab_base, krow_base, colp, tid);
                 if (tid == 0) s_next = 0;

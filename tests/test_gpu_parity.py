@@ -323,3 +323,36 @@ def test_host_buffer_entry_point(S):
     out = S.interaction_matrix_host(geom, torch.from_numpy(wl.cube).pin_memory(), wl.bbox, S.affines_of(wl))
     assert_parity(out.numpy().T.copy(), O.interaction_matrix(wl), wl)
     geom.destroy()
+
+
+def test_host_entry_point_packs_supports_edges_empty_modes_and_dense(S):
+    """With bboxes only the supports cross the bus (packed, per-mode origins): supports touching the grid
+    edge (origin -4), an all-zero mode, pageable memory, a repeated call on the same geometry; without
+    bboxes the whole cube goes (dense path)."""
+    import torch
+    wl = W.make_config(4, max_modes=40)           # 600-px grid, 60-px supports, some cut by the grid edge
+    rng = np.random.default_rng(5)
+    wl.cube[5] = 0
+    wl.bbox[5] = (0, 0, -1, -1)
+    wl.cube[6] = 0                                  # a support in the upper-left corner: packed origin (-4, -1)
+    wl.cube[6, 0:20, 0:17] = rng.uniform(0.1, 1.0, (20, 17)).astype(np.float32)
+    wl.bbox[6] = (0, 0, 16, 19)
+    wl.cube[7] = 0                                  # ... and one against the far edges
+    wl.cube[7, wl.ny - 31:, wl.nx - 25:] = rng.uniform(0.1, 1.0, (31, 25)).astype(np.float32)
+    wl.bbox[7] = (wl.nx - 25, wl.ny - 31, wl.nx - 1, wl.ny - 1)
+    ref = O.interaction_matrix(wl)
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    for _ in range(2):
+        out = S.interaction_matrix_host(geom, wl.cube, wl.bbox, S.affines_of(wl))      # numpy, pageable
+        assert_parity(out.numpy().T.copy(), ref, wl)
+    bad = wl.bbox.copy()
+    bad[0, 2] = wl.nx
+    with pytest.raises(S.SynimError) as e:
+        S.interaction_matrix_host(geom, wl.cube, bad, S.affines_of(wl))
+    assert e.value.status == S.ERR_INVALID_ARG
+    geom.destroy()
+    wl = W.make_config(5, max_modes=3)
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    out = S.interaction_matrix_host(geom, torch.from_numpy(wl.cube).pin_memory(), None, S.affines_of(wl))
+    assert_parity(out.numpy().T.copy(), O.interaction_matrix(wl), wl)
+    geom.destroy()

@@ -55,7 +55,7 @@ typedef enum {
     SYNIM_ERR_UNSUPPORTED_DEVICE = -4, /* current device is not compute capability 10.x */
     SYNIM_ERR_OUT_OF_MEMORY = -5,
     SYNIM_ERR_CUDA = -6,               /* any other CUDA runtime / driver failure */
-    SYNIM_ERR_UNSUPPORTED = -7         /* feature not built on this path (see synim_slope_mode) */
+    SYNIM_ERR_UNSUPPORTED = -7         /* reserved: a feature not built on this path (none at present) */
 } synim_status;
 
 /* Slope estimator.  ND = finite central differences averaged over the subaperture
@@ -128,7 +128,9 @@ int64_t synim_row_offset(const synim_geometry *geom, int32_t wfs);
  *   bbox_max_w/h HOST upper bounds of x1-x0+1 / y1-y0+1 over all modes, used only to size the
  *                shared-memory tiles (<= 0: unknown).  Wrong bounds cost speed, never correctness.
  *   affine       HOST [n_wfs]
- *   mode         SYNIM_SLOPES_ND; SYNIM_SLOPES_GTILT returns SYNIM_ERR_UNSUPPORTED on this build
+ *   mode         SYNIM_SLOPES_ND (the paper's engine) or SYNIM_SLOPES_GTILT (comparison estimator: same
+ *                kernel, the slopes are sums of phi weighted by the G-tilt coefficient maps built at
+ *                synim_create_geometry); anything else is INVALID_ARG
  *   d_out        DEVICE float32, column-major, ld >= synim_num_rows(); every element of rows
  *                [0, num_rows) of columns [0, n_modes) is written (padding rows are left untouched)
  * Errors: INVALID_ARG (NULL, n_modes < 0, ld < rows, singular affine), ALIGNMENT, CUDA. */

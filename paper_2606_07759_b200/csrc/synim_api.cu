@@ -46,6 +46,7 @@ struct WfsHost {
     int n_subap = 0, n_pix = 0, M = 0, n_valid = 0;
     int row_x = 0, row_y = 0;
     float *d_wmap = nullptr;
+    float *d_gx = nullptr, *d_gy = nullptr;   // G-tilt coefficient maps
     int *d_subap_row = nullptr;
 };
 
@@ -189,6 +190,8 @@ void synim_destroy(synim_geometry *g)
     if (!g) return;
     for (auto &w : g->wfs) {
         if (w.d_wmap) cudaFree(w.d_wmap);
+        if (w.d_gx) cudaFree(w.d_gx);
+        if (w.d_gy) cudaFree(w.d_gy);
         if (w.d_subap_row) cudaFree(w.d_subap_row);
     }
     if (g->ws_cube) cudaFree(g->ws_cube);
@@ -267,6 +270,13 @@ synim_status synim_create_geometry(int32_t ny, int32_t nx, int32_t n_wfs, const 
             return cleanup(cuda_fail(e, "cudaMemcpyAsync(valid)"));
         if ((e = synim::launch_subap_weights(grids[w].d_pupil, d_valid, h.n_subap, h.n_pix, h.d_wmap, d_err, s)) != cudaSuccess)
             return cleanup(cuda_fail(e, "subap_weights_kernel"));
+        // the G-tilt estimator's coefficient maps, same layout
+        if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_gx), wmap_bytes)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMalloc(gx)"));
+        if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_gy), wmap_bytes)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMalloc(gy)"));
+        if ((e = cudaMemsetAsync(h.d_gx, 0, wmap_bytes, s)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMemsetAsync(gx)"));
+        if ((e = cudaMemsetAsync(h.d_gy, 0, wmap_bytes, s)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMemsetAsync(gy)"));
+        if ((e = synim::launch_gtilt_maps(grids[w].d_pupil, d_valid, h.n_subap, h.n_pix, h.d_gx, h.d_gy, s)) != cudaSuccess)
+            return cleanup(cuda_fail(e, "gtilt_maps_kernel"));
         // d_valid is reused by the next sensor: stream order keeps this safe
     }
     g->rows = row;
@@ -301,9 +311,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
                                            void *stream)
 {
     if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
-    if (mode == SYNIM_SLOPES_GTILT)
-        return fail(SYNIM_ERR_UNSUPPORTED, "synim_interaction_matrix: the G-tilt telescoping sum is not built on the GPU path");
-    if (mode != SYNIM_SLOPES_ND) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: unknown slope mode %d", (int)mode);
+    if (mode != SYNIM_SLOPES_ND && mode != SYNIM_SLOPES_GTILT) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: unknown slope mode %d", (int)mode);
     if (n_modes == 0) return SYNIM_OK;
     if (!d_influence || !d_out) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL device buffer");
     if (ld < g->rows) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: ld = %lld < rows = %lld", (long long)ld, g->rows);
@@ -338,7 +346,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         synim::WfsDev &d = dev[w];
         if (!build_maps(affine[w], h.M, ny, nx, d.fwd, d.inv))
             return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: sensor %d: singular or non-finite affine", w);
-        d.wmap = h.d_wmap; d.subap_row = h.d_subap_row;
+        d.wmap = h.d_wmap; d.gx = h.d_gx; d.gy = h.d_gy; d.subap_row = h.d_subap_row;
         d.scale = (float)affine[w].slope_scale;
         d.M = h.M; d.n_subap = h.n_subap; d.n_pix = h.n_pix; d.row_x = h.row_x; d.row_y = h.row_y;
         d.tab_off = 0; d.tab_cap = 0;
@@ -400,7 +408,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
             const WfsHost &last = g->wfs[w0 + nw - 1];
             p.zero_count = last.row_x + 2 * last.n_valid - p.zero_begin;
         }
-        SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, s));
+        SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, mode == SYNIM_SLOPES_GTILT, s));
     }
     return SYNIM_OK;
 }

@@ -19,6 +19,7 @@ struct WfsDev {
     double fwd[6];
     double inv[6];
     const float *wmap;       // [M][M]  0.5*P/W_S, 0 where the subaperture is invalid
+    const float *gx, *gy;    // [M][M]  G-tilt coefficients (gtilt_maps_kernel); same rows of zeros below
     const int *subap_row;    // [n_subap^2] index among the valid subapertures, -1 if invalid
     float scale;             // slope_scale
     int M, n_subap, n_pix;
@@ -47,9 +48,11 @@ struct ImParams {
 // launchers; all asynchronous on `stream`, return the launch status.
 // The hot path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
 // {patch_pitch, patch_h, 1}
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream);
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
                                  float *d_wmap, int *d_error_flag, cudaStream_t stream);
+cudaError_t launch_gtilt_maps(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix, float *d_gx, float *d_gy,
+                              cudaStream_t stream);
 cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox, int *d_diag,
                                   cudaStream_t stream);
 cudaError_t launch_bbox_extent(const int *d_bbox, int n_modes, int *d_wh, cudaStream_t stream);

@@ -38,6 +38,54 @@ __global__ void __launch_bounds__(128) subap_weights_kernel(const float *__restr
     }
 }
 
+// G-tilt (reading R13) as two coefficient maps.  A pixel is valid iff
+// P >= 0.5.  For every pixel row of a subaperture with first / last valid columns jf < jl the estimator
+// adds phi[row][jl] - phi[row][jf] to a numerator and jl - jf to a denominator; s_x = num / den (0 if
+// den = 0), and the same over pixel columns for s_y.  That is s_x = sum gx*phi, s_y = sum gy*phi with
+// gx = +-1/den_x on those end pixels and 0 elsewhere.  One CTA per subaperture; gx, gy arrive zeroed.
+__global__ void __launch_bounds__(128) gtilt_maps_kernel(const float *__restrict__ pupil, const uint8_t *__restrict__ valid,
+                                                         int n_subap, int n_pix, float *__restrict__ gx,
+                                                         float *__restrict__ gy)
+{
+    __shared__ int den[2];
+    const int s = blockIdx.x, a = s / n_subap, b = s - a * n_subap;
+    if (!valid[s]) return;   // CTA-uniform
+    const int M = n_subap * n_pix, i0 = a * n_pix, j0 = b * n_pix;
+    if (threadIdx.x < 2) den[threadIdx.x] = 0;
+    __syncthreads();
+    // pass 1: the two denominators
+    for (int r = threadIdx.x; r < 2 * n_pix; r += 128) {
+        const int axis = r >= n_pix, q = axis ? r - n_pix : r;   // axis 0: pixel row i0+q; axis 1: pixel column j0+q
+        int f = -1, l = -1;
+        for (int t = 0; t < n_pix; ++t) {
+            const float pv = axis ? pupil[(size_t)(i0 + t) * M + j0 + q] : pupil[(size_t)(i0 + q) * M + j0 + t];
+            if (pv >= 0.5f) { if (f < 0) f = t; l = t; }
+        }
+        if (f >= 0 && l > f) atomicAdd(&den[axis], l - f);
+    }
+    __syncthreads();
+    // pass 2: +-1/den on the end pixels
+    for (int r = threadIdx.x; r < 2 * n_pix; r += 128) {
+        const int axis = r >= n_pix, q = axis ? r - n_pix : r;
+        if (den[axis] <= 0) continue;
+        int f = -1, l = -1;
+        for (int t = 0; t < n_pix; ++t) {
+            const float pv = axis ? pupil[(size_t)(i0 + t) * M + j0 + q] : pupil[(size_t)(i0 + q) * M + j0 + t];
+            if (pv >= 0.5f) { if (f < 0) f = t; l = t; }
+        }
+        if (f >= 0 && l > f) {
+            const float c = (float)(1.0 / (double)den[axis]);
+            if (axis) {
+                gy[(size_t)(i0 + l) * M + j0 + q] = c;
+                gy[(size_t)(i0 + f) * M + j0 + q] = -c;
+            } else {
+                gx[(size_t)(i0 + q) * M + j0 + l] = c;
+                gx[(size_t)(i0 + q) * M + j0 + f] = -c;
+            }
+        }
+    }
+}
+
 // one CTA per mode: tight non-zero extent (x0,y0,x1,y1) and, if asked for, the diagonal extents
 // (min x+y, max x+y, min x-y, max x-y) of the non-zero pixels: together the support's bounding octagon
 __global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ cube, int ny, int nx,
@@ -113,6 +161,13 @@ cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, i
 {
     subap_weights_kernel<<<n_subap * n_subap, 128, 0, stream>>>(d_pupil, d_valid, n_subap, n_pix, d_wmap,
                                                                 d_error_flag);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gtilt_maps(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix, float *d_gx, float *d_gy,
+                              cudaStream_t stream)
+{
+    gtilt_maps_kernel<<<n_subap * n_subap, 128, 0, stream>>>(d_pupil, d_valid, n_subap, n_pix, d_gx, d_gy);
     return cudaGetLastError();
 }
 

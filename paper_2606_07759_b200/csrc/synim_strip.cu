@@ -149,7 +149,8 @@ struct CellBox {
 
 // Everything a strip needs from its sensor, read once from the kernel parameters.
 struct StripSensor {
-    const float *wmap;
+    const float *wmap;    // weights of the x sums: 0.5*P/W_S, or gx
+    const float *wmap2;   // weights of the y sums: the same map, or gy
     int M, n_subap, n_pix;
 };
 
@@ -175,6 +176,10 @@ struct ZeroPacer {
 // One strip: D columns jA .. jA+nC-1 (lanes 1..nC), D rows i0 .. i1 of sensor W.
 // Its partial slopes are added to the CTA's shared table: entry (a, b, axis) of the sensor's window of
 // subapertures (first row a0, first column b0, nb columns) sits at tab + ((a-a0)*nb + (b-b0))*8 + axis*4.
+// kGtilt: the G-tilt estimator (reading R13) instead of the numerical derivative: the slopes are then two
+// weighted sums of phi itself (coefficient maps gx, gy: +-1/den on the first / last valid pixel of every
+// pixel row / column of a subaperture), so the stencil and its shuffles drop out.
+template <bool kGtilt>
 __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
                                               uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp)
 {
@@ -215,7 +220,8 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     if (d_hi < d_lo) return;
 
     StripSensor S;
-    S.wmap = W.wmap; S.M = W.M; S.n_subap = W.n_subap; S.n_pix = W.n_pix;
+    S.wmap = kGtilt ? W.gx : W.wmap; S.wmap2 = kGtilt ? W.gy : W.wmap;
+    S.M = W.M; S.n_subap = W.n_subap; S.n_pix = W.n_pix;
 
     // segments of lanes that belong to one subaperture column
     const int npx = S.n_pix;
@@ -301,9 +307,12 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     constexpr int kRows = kStripRows;
     float rf = (float)(d_lo + 1);
     float pmA = sample((float)(d_lo - 1)), pmB = sample((float)d_lo);   // phi[d-1], phi[d]
-    float wgt[kRows];
+    float wgt[kRows], wg2[kRows];
 #pragma unroll
-    for (int k = 0; k < kRows; ++k) wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
+    for (int k = 0; k < kRows; ++k) {
+        wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
+        wg2[k] = kGtilt ? __ldg(S.wmap2 + (woff + (uint32_t)k * wrow)) : wgt[k];
+    }
     float sx = 0.0f, sy = 0.0f;
 #pragma unroll(kStripUnroll)
     for (int d = d_lo; d <= d_hi; d += kRows) {
@@ -311,9 +320,12 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         for (int q = 0; q < (kComputeWarps >= 4 ? 1 : 4 / kComputeWarps); ++q) zp.step();
         // weights of the next kRows rows, one iteration ahead of their use
         woff += wstride;
-        float wnx[kRows];
+        float wnx[kRows], wn2[kRows];
 #pragma unroll
-        for (int k = 0; k < kRows; ++k) wnx[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
+        for (int k = 0; k < kRows; ++k) {
+            wnx[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
+            wn2[k] = kGtilt ? __ldg(S.wmap2 + (woff + (uint32_t)k * wrow)) : wnx[k];
+        }
 
         float cur[kRows];   // phi[d+1 .. d+kRows]
 #pragma unroll
@@ -326,23 +338,27 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         for (int k = 0; k < kRows; ++k) {
             const float mid = k == 0 ? pmB : cur[k - 1];                         // phi[d+k]
             const float above = k == 0 ? pmA : (k == 1 ? pmB : cur[k - 2]);     // phi[d+k-1]
-            dy[k] = cur[k] - above;
-            dx[k] = __shfl_down_sync(kFull, mid, 1) - __shfl_up_sync(kFull, mid, 1);
+            if (kGtilt) {
+                dx[k] = mid; dy[k] = mid;   // the sums run over phi itself
+            } else {
+                dy[k] = cur[k] - above;
+                dx[k] = __shfl_down_sync(kFull, mid, 1) - __shfl_up_sync(kFull, mid, 1);
+            }
         }
         if (rem + kRows < npx) {   // warp-uniform: no subaperture row ends inside these rows
 #pragma unroll
-            for (int k = 0; k < kRows; ++k) { sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wgt[k], dy[k], sy); }
+            for (int k = 0; k < kRows; ++k) { sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wg2[k], dy[k], sy); }
             rem += kRows;
         } else {
 #pragma unroll
             for (int k = 0; k < kRows; ++k) {
-                sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wgt[k], dy[k], sy);
+                sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wg2[k], dy[k], sy);
                 if (++rem == npx) { flush(sx, sy); sx = 0.0f; sy = 0.0f; rem = 0; }
             }
         }
         pmA = cur[kRows - 2]; pmB = cur[kRows - 1];
 #pragma unroll
-        for (int k = 0; k < kRows; ++k) wgt[k] = wnx[k];
+        for (int k = 0; k < kRows; ++k) { wgt[k] = wnx[k]; wg2[k] = wn2[k]; }
     }
     if (rem > 0) flush(sx, sy);
 }
@@ -376,6 +392,7 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
     }
 }
 
+template <bool kGtilt>
 __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
                                                                                      const __grid_constant__ CUtensorMap tmap)
 {
@@ -550,7 +567,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
                 const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
                 const int jA = j0 + (t - base) * kStripCols;
                 const int nC = min(kStripCols, j1 - jA + 1);
-                process_strip(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
+                process_strip<kGtilt>(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
             }
             if (multi) {
                 cp_async_wait_all();
@@ -575,14 +592,15 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
 
 }  // namespace
 
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, cudaStream_t stream)
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream)
 {
     if (p.n_modes <= 0) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(synim_strip_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    auto kernel = gtilt ? synim_strip_kernel<true> : synim_strip_kernel<false>;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     CUtensorMap tm;
     memcpy(&tm, tensor_map, sizeof(tm));
-    synim_strip_kernel<<<dim3((unsigned)p.n_modes, (unsigned)(p.chunks > 0 ? p.chunks : 1)), kStripThreads, smem_bytes, stream>>>(p, tm);
+    kernel<<<dim3((unsigned)p.n_modes, (unsigned)(p.chunks > 0 ? p.chunks : 1)), kStripThreads, smem_bytes, stream>>>(p, tm);
     return cudaGetLastError();
 }
 

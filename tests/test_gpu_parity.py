@@ -300,6 +300,31 @@ def test_wfs_looking_past_the_source_grid_and_strong_magnification(S):
     assert_parity(gpu_im(S, wl, hint=False), ref, wl)
 
 
+def test_full_physical_chain_and_degenerate_sensor_grids(S):
+    """Every parameter of the composite matrix at once (DM shift / rotation / magnification, cone effect,
+    off-axis footprint, sub-pixel alignment scale s != 1), sensors with one pixel per subaperture and with
+    a single subaperture, both estimators, zonal and dense."""
+    ny, nx = 64, 64
+    cube = W.random_smooth_cube(5, ny, nx, 77)
+    sensors = []
+    for n_subap, n_pix, phys in (
+            (8, 6, W.physical(shift_x=0.4, shift_y=-0.7, rot_deg=12.0, mag_x=1.03, mag_y=0.98, dm_shift_x=-1.3,
+                              dm_shift_y=0.6, dm_rot_deg=-4.0, dm_mag=1.05, dm_height_m=9000.0, gs_range_m=90000.0,
+                              gs_theta_arcsec=20.0, gs_azimuth_deg=40.0, src_pixel_pitch_m=0.35, wfs_pitch_src_px=1.1)),
+            (40, 1, W.physical(rot_deg=-20.0, shift_x=1.5)),          # one pixel per subaperture
+            (1, 44, W.physical(rot_deg=5.0, mag_x=1.1, mag_y=1.1))):  # a single subaperture
+        m = n_subap * n_pix
+        pup = W.make_pupil(m, float(m), 0.0) if n_subap > 1 else np.ones((m, m), np.float32)
+        sensors.append(W.WfsInput(n_subap, n_pix, pup, W.valid_subaps(pup, n_subap, n_pix), phys))
+    wl = W.Workload("chain", 0, ny, nx, cube, None, sensors)
+    for mode, omode in ((S.SLOPES_ND, O.ND), (S.SLOPES_GTILT, O.GTILT)):
+        ref = O.interaction_matrix(wl, mode=omode)
+        wl.bbox = None
+        assert_parity(gpu_im(S, wl, mode=mode), ref, wl)
+        wl.bbox = W.tight_bboxes(cube)
+        assert_parity(gpu_im(S, wl, mode=mode), ref, wl)
+
+
 def test_compute_bboxes_matches_the_generator(S):
     import torch
     wl = W.make_config(2, max_modes=40)

@@ -364,6 +364,101 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
 }
 
 
+// Lane w of one warp: footprint of a piece (source pixels qx0..qx1 x qy0..qy1 of a support with diagonal
+// extents sg0..sg1, dg0..dg1) on sensor w.  phi(i,j) can be non-zero only strictly inside the image, under
+// the inverse map, of the piece's open octagon: the box (qx0-1,qx1+1)x(qy0-1,qy1+1) cut by
+// sg0-2 < x+y < sg1+2 and dg0-2 < x-y < dg1+2.  So D(i,j) only for floor(jmin) <= j <= ceil(jmax) (one pixel
+// of stencil either side), clipped to the sensor.  Results go to shared memory for the other warps.
+__device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, int qx0, int qx1, int qy0, int qy1, int sg0,
+                                                   int sg1, int dg0, int dg1, int4 *s_box, int4 *s_win)
+{
+        int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_a0 = 0, r_b0 = 0, r_na = 0, r_nb = 0;
+        const WfsDev &W = p.wfs[lane];
+        const double X0 = qx0 - 1, X1 = qx1 + 1, Y0 = qy0 - 1, Y1 = qy1 + 1;
+        const double S0 = sg0 - 2, S1 = sg1 + 2, D0 = dg0 - 2, D1 = dg1 + 2;
+        double jmin = 1e300, jmax = -1e300, imin = 1e300, imax = -1e300;
+        auto vertex = [&](double c, double r) {
+            const double j = W.inv[0] * c + W.inv[1] * r + W.inv[2];
+            const double i = W.inv[3] * c + W.inv[4] * r + W.inv[5];
+            jmin = fmin(jmin, j); jmax = fmax(jmax, j); imin = fmin(imin, i); imax = fmax(imax, i);
+        };
+        // two vertices on each edge of the box; an edge the diagonals cut away altogether yields two
+        // points outside the octagon but inside the box (a superset: still exact)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const double X = e ? X1 : X0, Y = e ? Y1 : Y0;
+            const double ya = fmax(fmax(Y0, S0 - X), X - D1), yb = fmin(fmin(Y1, S1 - X), X - D0);
+            vertex(X, ya); vertex(X, yb);
+            const double xa = fmax(fmax(X0, S0 - Y), D0 + Y), xb = fmin(fmin(X1, S1 - Y), D1 + Y);
+            vertex(xa, Y); vertex(xb, Y);
+        }
+        const double lim = 1.0e9;
+        r_j0 = max(0, (int)floor(fmax(jmin, -lim))); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)));
+        r_i0 = max(0, (int)floor(fmax(imin, -lim))); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)));
+        int4 win = make_int4(0, 0, 0, 0);
+        if (r_j1 >= r_j0 && r_i1 >= r_i0) {
+            r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
+            r_nb = r_j1 / W.n_pix - r_b0 + 1;
+            r_na = r_i1 / W.n_pix - r_a0 + 1;
+            win = make_int4(r_a0, r_b0, r_na, r_nb);
+            if (win.z * win.w * 2 > W.tab_cap) __trap();   // the host sized the table from the same bounds
+        }
+        s_box[lane] = make_int4(r_i0, r_i1, r_j0, r_j1);
+        s_win[lane] = win;   // also read by scatter_table
+}
+
+// All warps, after a barrier: fetch the IM rows of the windows' subapertures (needed only when the table
+// is stored: asynchronously, so that the store at the end waits for nothing), then sample the strips of
+// every sensor's footprint.
+template <bool kGtilt>
+__device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, int lane, const int4 *s_box, const int4 *s_win,
+                                                  int *s_next_ptr, const CellBox &cb, uint32_t tab_base, uint32_t krow_base,
+                                                  ZeroPacer &zp)
+{
+    int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_nb = 0;
+    if (lane < p.n_wfs) {
+        const int4 fb = s_box[lane], fw = s_win[lane];
+        r_i0 = fb.x; r_i1 = fb.y; r_j0 = fb.z; r_j1 = fb.w;
+        r_a0 = fw.x; r_b0 = fw.y; r_nb = fw.w;
+        if (r_j1 >= r_j0 && r_i1 >= r_i0) r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
+    }
+    // the IM rows of the windows' subapertures, needed only when the table is stored: fetched now,
+    // asynchronously, so that the store at the end waits for nothing (sensor w by warp w mod 4)
+    for (int w = warp; w < p.n_wfs; w += kComputeWarps) {
+        const int4 fw = s_win[w];   // a0, b0, na, nb
+        const WfsDev &W = p.wfs[w];
+        const int n = fw.z * fw.w;
+        const unsigned magic = 0xFFFFFFFFu / (unsigned)max(fw.w, 1) + 1u;   // (wraps to 0 for 1)
+        for (int e = lane; e < n; e += 32) {
+            const int ra = fw.w == 1 ? e : (int)__umulhi((unsigned)e, magic), rb = e - ra * fw.w;
+            cp_async_4(krow_base + (uint32_t)((W.tab_off >> 1) + e) * 4u, W.subap_row + (fw.x + ra) * W.n_subap + (fw.y + rb));
+        }
+    }
+    int incl = r_n;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int t = __shfl_up_sync(kFull, incl, d);
+        if (lane >= d) incl += t;
+    }
+    const int total = __shfl_sync(kFull, incl, 31);
+    // strips are handed out first come, first served: their costs differ (a strip over the rim of a
+    // round support has fewer live rows), and the CTA ends with its slowest warp
+    while (true) {
+        int t = 0;
+        if (lane == 0) t = atomicAdd(s_next_ptr, 1);
+        t = __shfl_sync(kFull, t, 0);
+        if (t >= total) break;
+        const int w = __popc(__ballot_sync(kFull, incl <= t));
+        const int base = __shfl_sync(kFull, incl - r_n, w);
+        const int i0 = __shfl_sync(kFull, r_i0, w), i1 = __shfl_sync(kFull, r_i1, w);
+        const int j0 = __shfl_sync(kFull, r_j0, w), j1 = __shfl_sync(kFull, r_j1, w);
+        const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
+        const int jA = j0 + (t - base) * kStripCols;
+        const int nC = min(kStripCols, j1 - jA + 1);
+        process_strip<kGtilt>(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
+    }
+}
+
 // The table's non-zero entries -> the IM column (S4).  kAtomic: the support was split into pieces, whose
 // contributions add up (linearity); the entries are cleared for the next piece.
 template <bool kAtomic, int NT>
@@ -380,11 +475,11 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
             const float v = lds_f32(tb + (uint32_t)e * 4u);
             if (v == 0.0f) continue;
             const int k = lds_s32(krow_base + (uint32_t)((W.tab_off >> 1) + (e >> 1)) * 4u);   // fetched while the strips ran
+            if (kAtomic) sts_f32(tb + (uint32_t)e * 4u, 0.0f);
             if (k < 0) continue;
             float *dst = colp + ((e & 1) ? W.row_y : W.row_x) + k;
             if (kAtomic) {
                 atomicAdd(dst, v * W.scale);
-                sts_f32(tb + (uint32_t)e * 4u, 0.0f);
             } else {
                 *dst = v * W.scale;
             }
@@ -476,45 +571,8 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             cb.pitchf = p.patch_pitchf;
             cb.s_lo = (float)(sg0 - 2 - (cb.x0 + cb.y0)) - 0.01f; cb.s_hi = (float)(sg1 + 2 - (cb.x0 + cb.y0)) + 0.01f;
             cb.d_lo = (float)(dg0 - 2 - (cb.x0 - cb.y0)) - 0.01f; cb.d_hi = (float)(dg1 + 2 - (cb.x0 - cb.y0)) + 0.01f;
-            // lane w: footprint of this piece on sensor w.  phi(i,j) can be non-zero only strictly inside the
-            // image, under the inverse map, of the piece's open octagon: the box (qx0-1,qx1+1)x(qy0-1,qy1+1)
-            // cut by sg0-2 < x+y < sg1+2 and dg0-2 < x-y < dg1+2.  So D(i,j) only for floor(jmin) <= j <=
-            // ceil(jmax) (one pixel of stencil either side), clipped to the sensor.
-            if (warp == 0 && lane < p.n_wfs) {   // once per CTA, while the box is still in flight
-                int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_a0 = 0, r_b0 = 0, r_na = 0, r_nb = 0;
-                const WfsDev &W = p.wfs[lane];
-                const double X0 = qx0 - 1, X1 = qx1 + 1, Y0 = qy0 - 1, Y1 = qy1 + 1;
-                const double S0 = sg0 - 2, S1 = sg1 + 2, D0 = dg0 - 2, D1 = dg1 + 2;
-                double jmin = 1e300, jmax = -1e300, imin = 1e300, imax = -1e300;
-                auto vertex = [&](double c, double r) {
-                    const double j = W.inv[0] * c + W.inv[1] * r + W.inv[2];
-                    const double i = W.inv[3] * c + W.inv[4] * r + W.inv[5];
-                    jmin = fmin(jmin, j); jmax = fmax(jmax, j); imin = fmin(imin, i); imax = fmax(imax, i);
-                };
-                // two vertices on each edge of the box; an edge the diagonals cut away altogether yields two
-                // points outside the octagon but inside the box (a superset: still exact)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const double X = e ? X1 : X0, Y = e ? Y1 : Y0;
-                    const double ya = fmax(fmax(Y0, S0 - X), X - D1), yb = fmin(fmin(Y1, S1 - X), X - D0);
-                    vertex(X, ya); vertex(X, yb);
-                    const double xa = fmax(fmax(X0, S0 - Y), D0 + Y), xb = fmin(fmin(X1, S1 - Y), D1 + Y);
-                    vertex(xa, Y); vertex(xb, Y);
-                }
-                const double lim = 1.0e9;
-                r_j0 = max(0, (int)floor(fmax(jmin, -lim))); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)));
-                r_i0 = max(0, (int)floor(fmax(imin, -lim))); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)));
-                int4 win = make_int4(0, 0, 0, 0);
-                if (r_j1 >= r_j0 && r_i1 >= r_i0) {
-                    r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
-                    r_nb = r_j1 / W.n_pix - r_b0 + 1;
-                    r_na = r_i1 / W.n_pix - r_a0 + 1;
-                    win = make_int4(r_a0, r_b0, r_na, r_nb);
-                    if (win.z * win.w * 2 > W.tab_cap) __trap();   // the host sized the table from the same bounds
-                }
-                s_box[lane] = make_int4(r_i0, r_i1, r_j0, r_j1);
-                s_win[lane] = win;   // also read by scatter_table
-            }
+            if (warp == 0 && lane < p.n_wfs)   // once per CTA, while the box is still in flight
+                footprint_of_piece(p, lane, qx0, qx1, qy0, qy1, sg0, sg1, dg0, dg1, s_box, s_win);
             mbar_wait(&bar, parity);
             parity ^= 1u;
 
@@ -527,48 +585,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             }
             bar_sync(1, kComputeThreads);   // footprints (and a cleared ring) visible
 
-            int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_nb = 0;
-            if (lane < p.n_wfs) {
-                const int4 fb = s_box[lane], fw = s_win[lane];
-                r_i0 = fb.x; r_i1 = fb.y; r_j0 = fb.z; r_j1 = fb.w;
-                r_a0 = fw.x; r_b0 = fw.y; r_nb = fw.w;
-                if (r_j1 >= r_j0 && r_i1 >= r_i0) r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
-            }
-            // the IM rows of the windows' subapertures, needed only when the table is stored: fetched now,
-            // asynchronously, so that the store at the end waits for nothing (sensor w by warp w mod 4)
-            for (int w = warp; w < p.n_wfs; w += kComputeWarps) {
-                const int4 fw = s_win[w];   // a0, b0, na, nb
-                const WfsDev &W = p.wfs[w];
-                const int n = fw.z * fw.w;
-                const unsigned magic = 0xFFFFFFFFu / (unsigned)max(fw.w, 1) + 1u;   // (wraps to 0 for 1)
-                for (int e = lane; e < n; e += 32) {
-                    const int ra = fw.w == 1 ? e : (int)__umulhi((unsigned)e, magic), rb = e - ra * fw.w;
-                    cp_async_4(krow_base + (uint32_t)((W.tab_off >> 1) + e) * 4u, W.subap_row + (fw.x + ra) * W.n_subap + (fw.y + rb));
-                }
-            }
-            int incl = r_n;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int t = __shfl_up_sync(kFull, incl, d);
-                if (lane >= d) incl += t;
-            }
-            const int total = __shfl_sync(kFull, incl, 31);
-            // strips are handed out first come, first served: their costs differ (a strip over the rim of a
-            // round support has fewer live rows), and the CTA ends with its slowest warp
-            while (true) {
-                int t = 0;
-                if (lane == 0) t = atomicAdd(&s_next, 1);
-                t = __shfl_sync(kFull, t, 0);
-                if (t >= total) break;
-                const int w = __popc(__ballot_sync(kFull, incl <= t));
-                const int base = __shfl_sync(kFull, incl - r_n, w);
-                const int i0 = __shfl_sync(kFull, r_i0, w), i1 = __shfl_sync(kFull, r_i1, w);
-                const int j0 = __shfl_sync(kFull, r_j0, w), j1 = __shfl_sync(kFull, r_j1, w);
-                const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
-                const int jA = j0 + (t - base) * kStripCols;
-                const int nC = min(kStripCols, j1 - jA + 1);
-                process_strip<kGtilt>(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
-            }
+            sample_footprints<kGtilt>(p, warp, lane, s_box, s_win, &s_next, cb, tab_base, krow_base, zp);
             if (multi) {
                 cp_async_wait_all();
                 bar_sync(1, kComputeThreads);   // every warp is done with this box and this piece's table

@@ -350,6 +350,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         d.scale = (float)affine[w].slope_scale;
         d.M = h.M; d.n_subap = h.n_subap; d.n_pix = h.n_pix; d.row_x = h.row_x; d.row_y = h.row_y;
         d.tab_off = 0; d.tab_cap = 0;
+        d.npx_magic = (unsigned)((0x100000000ULL + (unsigned long long)h.n_pix - 1) / (unsigned long long)h.n_pix);   // (unused for 1)
     }
     // per sensor a table of (x, y) partial slopes over the window of subapertures one piece's footprint
     // can span (the kernel derives the window from the same bounds and traps if it ever needed more)

@@ -23,6 +23,7 @@ struct WfsDev {
     const int *subap_row;    // [n_subap^2] index among the valid subapertures, -1 if invalid
     float scale;             // slope_scale
     int M, n_subap, n_pix;
+    unsigned npx_magic;      // ceil(2^32 / n_pix): x / n_pix = umulhi(x, npx_magic) for the pixel indices met here
     int row_x, row_y;        // first row of the x / y slopes of this sensor inside a column
     int tab_off, tab_cap;    // this sensor's slice of the CTA's slope table (floats)
 };

@@ -173,6 +173,10 @@ struct ZeroPacer {
     __device__ __forceinline__ bool pending() const { return next < end; }
 };
 
+// x / n_pix for 0 <= x < 2^15 without the integer-division sequence: magic = ceil(2^32 / n_pix) (exact while
+// x * n_pix < 2^32; n_pix = 1 would need 2^32 itself)
+__device__ __forceinline__ int div_npx(int x, int npx, unsigned magic) { return npx == 1 ? x : (int)__umulhi((unsigned)x, magic); }
+
 // One strip: D columns jA .. jA+nC-1 (lanes 1..nC), D rows i0 .. i1 of sensor W.
 // Its partial slopes are added to the CTA's shared table: entry (a, b, axis) of the sensor's window of
 // subapertures (first row a0, first column b0, nb columns) sits at tab + ((a-a0)*nb + (b-b0))*8 + axis*4.
@@ -226,7 +230,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // segments of lanes that belong to one subaperture column
     const int npx = S.n_pix;
     const bool isD = lane >= 1 && lane <= nC;
-    const int seg = isD ? jcol / npx : -1;
+    const int seg = isD ? div_npx(jcol, npx, W.npx_magic) : -1;
     const int segL = __shfl_up_sync(kFull, seg, 1);
     const bool head = isD && (lane == 1 || segL != seg);
     unsigned okm = 0;
@@ -237,7 +241,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     }
 
     const int i_first = i0 - 1 + d_lo;           // absolute row of D row d_lo
-    int a_cur = i_first / npx;
+    int a_cur = div_npx(i_first, npx, W.npx_magic);
     int rem = i_first - a_cur * npx;             // rows of subaperture row a_cur already behind us
     const int M = S.M;
     // weight map offsets (elements).  The map has kWmapPadRows rows of zeros below row M-1: halo lanes stay

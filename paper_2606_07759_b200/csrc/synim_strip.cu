@@ -322,15 +322,6 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     for (int d = d_lo; d <= d_hi; d += kRows) {
 #pragma unroll
         for (int q = 0; q < (kComputeWarps >= 4 ? 1 : 4 / kComputeWarps); ++q) zp.step();
-        // weights of the next kRows rows, one iteration ahead of their use
-        woff += wstride;
-        float wnx[kRows], wn2[kRows];
-#pragma unroll
-        for (int k = 0; k < kRows; ++k) {
-            wnx[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
-            wn2[k] = kGtilt ? __ldg(S.wmap2 + (woff + (uint32_t)k * wrow)) : wnx[k];
-        }
-
         float cur[kRows];   // phi[d+1 .. d+kRows]
 #pragma unroll
         for (int k = 0; k < kRows; ++k) cur[k] = sample(rf + (float)k);
@@ -361,8 +352,14 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
             }
         }
         pmA = cur[kRows - 2]; pmB = cur[kRows - 1];
+        // the weights of the next kRows rows, loaded into the registers just consumed: nothing touches them
+        // until the end of the next iteration (a register-to-register copy would wait for the load)
+        woff += wstride;
 #pragma unroll
-        for (int k = 0; k < kRows; ++k) { wgt[k] = wnx[k]; wg2[k] = wn2[k]; }
+        for (int k = 0; k < kRows; ++k) {
+            wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
+            wg2[k] = kGtilt ? __ldg(S.wmap2 + (woff + (uint32_t)k * wrow)) : wgt[k];
+        }
     }
     if (rem > 0) flush(sx, sy);
 }

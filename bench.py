@@ -230,6 +230,7 @@ def main():
         sampler.start()
         time.sleep(0.15)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    step()   # one more untimed step: the GPU sat idle while the clock sampler started
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()

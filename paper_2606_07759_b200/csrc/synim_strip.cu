@@ -614,8 +614,17 @@ cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_
 {
     if (p.n_modes <= 0) return cudaSuccess;
     auto kernel = gtilt ? synim_strip_kernel<true> : synim_strip_kernel<false>;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    // the opt-in shared-memory limit only ever has to grow (per device; a race sets it twice, harmlessly)
+    static size_t granted[2][64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
+    size_t &have = granted[gtilt ? 1 : 0][dev & 63];
+    if (smem_bytes > have) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return e;
+        have = smem_bytes;
+    }
     CUtensorMap tm;
     memcpy(&tm, tensor_map, sizeof(tm));
     kernel<<<dim3((unsigned)p.n_modes, (unsigned)(p.chunks > 0 ? p.chunks : 1)), kStripThreads, smem_bytes, stream>>>(p, tm);

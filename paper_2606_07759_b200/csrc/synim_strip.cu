@@ -1,6 +1,7 @@
-// synim_strip.cu -- the compact-support ("zonal") interaction-matrix kernel for sm_100a.
+// synim_strip.cu -- the interaction-matrix kernel for sm_100a (S1-S4 of SURVEY.md sec. 8(a)).
 //
-// One CTA per mode.  The mode's support (its bbox plus the one-pixel ring a bilinear sample can still
+// Compact-support ("zonal") modes: one CTA per mode.  (Dense modes: the whole grid cut into pieces, several
+// CTAs per mode -- see the kernel; G-tilt instead of the numerical derivative -- see process_strip.)  The mode's support (its bbox plus the one-pixel ring a bilinear sample can still
 // touch) is staged ONCE in shared memory by a TMA 3-D box load (cp.async.bulk.tensor, out-of-range
 // elements zero-filled by the hardware = reading R4) and reused by every sensor of the batch
 // (the cube is fetched once for all WFS).  Each warp then takes "strips": 30 WFS pixel
@@ -33,22 +34,23 @@ namespace synim {
 
 namespace {
 
-#ifndef SYNIM_STRIP_UNROLL
-#define SYNIM_STRIP_UNROLL 1
-#endif
+// Build parameters (measured on B200: these values are the fastest at config 3)
 #ifndef SYNIM_STRIP_WARPS
-#define SYNIM_STRIP_WARPS 4
+#define SYNIM_STRIP_WARPS 4    // warps per CTA
+#endif
+#ifndef SYNIM_STRIP_MINB
+#define SYNIM_STRIP_MINB 7     // CTAs per SM the register allocation aims at (72 registers)
+#endif
+#ifndef SYNIM_STRIP_ROWS
+#define SYNIM_STRIP_ROWS 2     // pixel rows per loop iteration (independent samples in flight per lane)
+#endif
+#ifndef SYNIM_STRIP_UNROLL
+#define SYNIM_STRIP_UNROLL 1   // unrolling of the row loop
 #endif
 constexpr int kComputeWarps = SYNIM_STRIP_WARPS, kComputeThreads = 32 * kComputeWarps;
 constexpr int kStripThreads = kComputeThreads;
-#ifndef SYNIM_STRIP_MINB
-#define SYNIM_STRIP_MINB 7
-#endif
-#ifndef SYNIM_STRIP_ROWS
-#define SYNIM_STRIP_ROWS 2
-#endif
 constexpr int kStripUnroll = SYNIM_STRIP_UNROLL;
-constexpr int kStripRows = SYNIM_STRIP_ROWS;                // pixel rows per loop iteration (independent samples in flight per lane)
+constexpr int kStripRows = SYNIM_STRIP_ROWS;
 static_assert(2 * kStripRows <= kWmapPadRows, "weight look-ahead runs past the rows of zeros");
 constexpr int kStripCols = 30;               // D columns per strip: lanes 1..30, halo on lanes 0 and 31
 constexpr float kMagicFloor = 12582912.0f;   // 1.5 * 2^23: fadd.rm(x, magic) = magic + floor(x), |x| < 2^22

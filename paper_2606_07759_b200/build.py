@@ -36,16 +36,18 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False, extra=()) -> str:
-    """Compile csrc/*.cu into paper_2606_07759_b200/libsynim.so; returns its path."""
-    if not force and not stale():
+def build_library(force: bool = False, verbose: bool = False, extra=(), out: str = LIB) -> str:
+    """Compile csrc/*.cu into paper_2606_07759_b200/libsynim.so (or ``out``); returns its path.
+    ``extra=("-DSYNIM_CHECKS",)`` gives the debug build whose kernels trap on any shared-memory, weight-map
+    or slope-table access outside its bounds."""
+    if out == LIB and not force and not stale():
         return LIB
-    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-o", out] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd), file=sys.stderr)
     subprocess.check_call(cmd)
-    return LIB
+    return out
 
 
 if __name__ == "__main__":

@@ -144,6 +144,7 @@ struct CellBox {
     uint32_t base;   // shared-window byte address of pixel (x0, y0) in the staged box
     int pitch;       // floats per row of the staged box
     float pitchf;    // the same, as float
+    uint32_t limit;  // end of the staged box (debug checks only)
     // a sample can be non-zero only for s_lo < col+row < s_hi and d_lo < col-row < d_hi as well (the
     // support's bounding octagon, grown by the reach of a bilinear sample)
     float s_lo, s_hi, d_lo, d_hi;
@@ -263,6 +264,9 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
             if ((m >> s) & 1u) { sx += tx; sy += ty; }
         }
         if (head && (sx != 0.0f || sy != 0.0f) && a_cur < S.n_subap) {
+#ifdef SYNIM_CHECKS
+            if (tent < tab || tent + 8u > tab + (uint32_t)W.tab_cap * 4u) __trap();
+#endif
             red_shared_f32(tent, sx);   // another warp may hold the other columns of this subaperture
             red_shared_f32(tent + 4u, sy);
         }
@@ -287,6 +291,10 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         // magic + c0 + r0*pitch is exact: its mantissa is the element index
         const uint32_t idx = __float_as_uint(fmaf(tr - kMagicFloor, pitchf, tc));
         const uint32_t at = idx * 4u + cbase;
+#ifdef SYNIM_CHECKS   // debug build: a sample that passes the range test must lie inside the staged box
+        if (__float_as_uint(col) < cw_bits && __float_as_uint(row) < ch_bits &&
+            (at < cb.base || at + rpitch4 + 8u > cb.limit)) __trap();
+#endif
         float phi;
         asm volatile(
             "{\n\t.reg .pred p;\n\t.reg .f32 v00, v01, v10, v11, t, u;\n\t.reg .b32 at1;\n\t"
@@ -313,9 +321,16 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     constexpr int kRows = kStripRows;
     float rf = (float)(d_lo + 1);
     float pmA = sample((float)(d_lo - 1)), pmB = sample((float)d_lo);   // phi[d-1], phi[d]
+#ifdef SYNIM_CHECKS
+    const uint32_t wlimit = (uint32_t)(M + kWmapPadRows) * (uint32_t)M;
+#define SYNIM_WCHECK(o) do { if ((o) >= wlimit) __trap(); } while (0)
+#else
+#define SYNIM_WCHECK(o) do { } while (0)
+#endif
     float wgt[kRows], wg2[kRows];
 #pragma unroll
     for (int k = 0; k < kRows; ++k) {
+        SYNIM_WCHECK(woff + (uint32_t)k * wrow);
         wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
         wg2[k] = kGtilt ? __ldg(S.wmap2 + (woff + (uint32_t)k * wrow)) : wgt[k];
     }
@@ -359,7 +374,8 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         woff += wstride;
 #pragma unroll
         for (int k = 0; k < kRows; ++k) {
-            wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
+            SYNIM_WCHECK(woff + (uint32_t)k * wrow);
+        wgt[k] = __ldg(S.wmap + (woff + (uint32_t)k * wrow));
             wg2[k] = kGtilt ? __ldg(S.wmap2 + (woff + (uint32_t)k * wrow)) : wgt[k];
         }
     }
@@ -572,6 +588,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             cb.base = raw_base + (uint32_t)slack * 4u;
             cb.pitch = p.patch_pitch;
             cb.pitchf = p.patch_pitchf;
+            cb.limit = raw_base + (uint32_t)(p.patch_pitch * p.patch_h) * 4u;
             cb.s_lo = (float)(sg0 - 2 - (cb.x0 + cb.y0)) - 0.01f; cb.s_hi = (float)(sg1 + 2 - (cb.x0 + cb.y0)) + 0.01f;
             cb.d_lo = (float)(dg0 - 2 - (cb.x0 - cb.y0)) - 0.01f; cb.d_hi = (float)(dg1 + 2 - (cb.x0 - cb.y0)) + 0.01f;
             if (warp == 0 && lane < p.n_wfs)   // once per CTA, while the box is still in flight

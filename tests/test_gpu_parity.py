@@ -325,6 +325,24 @@ def test_full_physical_chain_and_degenerate_sensor_grids(S):
         assert_parity(gpu_im(S, wl, mode=mode), ref, wl)
 
 
+def test_debug_build_traps_on_nothing(S, tmp_path):
+    """The -DSYNIM_CHECKS build traps on any shared-memory, weight-map or slope-table access outside its
+    bounds; every launch configuration runs through it cleanly (compute-sanitizer is closed on this pool)."""
+    from paper_2606_07759_b200 import build
+    lib = build.build_library(extra=("-DSYNIM_CHECKS",), out=str(tmp_path / "libsynim_checks.so"))
+    saved = (S.LIB_PATH, S._lib)
+    S.LIB_PATH, S._lib = lib, None
+    try:
+        for cfg, n, kw in ((1, None, {}), (1, None, dict(hint=False)), (1, None, dict(use_bbox=False)),
+                           (1, None, dict(mode=S.SLOPES_GTILT)), (3, 24, {}), (4, 16, {}), (4, 8, dict(hint=False)),
+                           (5, 1, {})):
+            wl = W.make_config(cfg, max_modes=n)
+            got = gpu_im(S, wl, **kw)
+            assert np.isfinite(got).all()
+    finally:
+        S.LIB_PATH, S._lib = saved
+
+
 def test_compute_bboxes_matches_the_generator(S):
     import torch
     wl = W.make_config(2, max_modes=40)

@@ -340,7 +340,12 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
     }
     const int cap_w = patch_pitch - 5, cap_h = patch_h - 2;
 
-    std::vector<synim::WfsDev> dev(n_wfs);
+    std::vector<synim::WfsDev> dev;
+    try {
+        dev.resize(n_wfs);
+    } catch (...) {
+        return fail(SYNIM_ERR_OUT_OF_MEMORY, "synim_interaction_matrix: host allocation failed");
+    }
     for (int w = 0; w < n_wfs; ++w) {
         const WfsHost &h = g->wfs[w];
         synim::WfsDev &d = dev[w];
@@ -522,14 +527,21 @@ synim_status synim_interaction_matrix_host(const synim_geometry *g, const float 
             }
         };
         const int nthreads = (int)std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
-        if (nthreads == 1 || n_modes < 64) {
-            pack(0, n_modes);
-        } else {
+        int done = 0;   // modes [0, done) are packed (or handed to a thread)
+        if (nthreads > 1 && n_modes >= 64) {
             std::vector<std::thread> pool;
-            for (int t = 0; t < nthreads; ++t)
-                pool.emplace_back(pack, (int)((long long)n_modes * t / nthreads), (int)((long long)n_modes * (t + 1) / nthreads));
+            try {   // no exception crosses the C ABI: what the threads could not be started for is packed here
+                pool.reserve(nthreads);
+                for (int t = 0; t < nthreads; ++t) {
+                    const int m1 = (int)((long long)n_modes * (t + 1) / nthreads);
+                    pool.emplace_back(pack, done, m1);
+                    done = m1;
+                }
+            } catch (...) {
+            }
             for (auto &th : pool) th.join();
         }
+        pack(done, n_modes);
         SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, stage, cube_bytes, cudaMemcpyHostToDevice, s));
         SYNIM_CUDA(cudaMemcpyAsync(g->ws_bbox, meta, meta_bytes, cudaMemcpyHostToDevice, s));
         st = run_interaction_matrix(g, g->ws_cube, pny, pnx, g->ws_bbox + 4 * (size_t)n_modes, n_modes, g->ws_bbox, nullptr, bw, bh,

@@ -164,6 +164,9 @@ synim_status synim_interaction_matrix_host(const synim_geometry *geom, const flo
 void synim_destroy(synim_geometry *geom); /* NULL-safe; frees the internal device buffers */
 const char *synim_last_error(void);       /* thread-local, never NULL */
 int32_t synim_version(void);              /* major*1000 + minor */
+/* Number of CUDA kernels this library has launched in this process so far (all entry points, all threads);
+ * bench.py reports the difference around its timed steps as gpu_launches. */
+int64_t synim_launch_count(void);
 
 #ifdef __cplusplus
 }

@@ -150,6 +150,8 @@ const char *synim_last_error(void) { return g_err; }
 
 int32_t synim_version(void) { return SYNIM_VERSION_MAJOR * 1000 + SYNIM_VERSION_MINOR; }
 
+int64_t synim_launch_count(void) { return (int64_t)synim::launches_so_far(); }
+
 synim_status synim_compose_affine(const synim_wfs_physical *p, synim_wfs_affine *out)
 {
     if (!p || !out) return fail(SYNIM_ERR_INVALID_ARG, "synim_compose_affine: NULL argument");
@@ -313,6 +315,12 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
     if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
     if (mode != SYNIM_SLOPES_ND && mode != SYNIM_SLOPES_GTILT) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: unknown slope mode %d", (int)mode);
     if (n_modes == 0) return SYNIM_OK;
+    {   // the geometry's buffers live on the device it was created on (an sm_100 one: checked there)
+        int cur = -1;
+        SYNIM_CUDA(cudaGetDevice(&cur));
+        if (cur != g->device)
+            return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: current device %d is not the geometry's device %d", cur, g->device);
+    }
     if (!d_influence || !d_out) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL device buffer");
     if (ld < g->rows) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: ld = %lld < rows = %lld", (long long)ld, g->rows);
     if (reinterpret_cast<uintptr_t>(d_influence) % 16 != 0)
@@ -449,13 +457,20 @@ synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *
     if (n_modes == 0) return SYNIM_OK;
     if (!d_bbox) return fail(SYNIM_ERR_INVALID_ARG, "synim_bbox_extent: NULL device buffer");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    int *d_wh = nullptr;
-    SYNIM_CUDA(cudaMalloc(reinterpret_cast<void **>(&d_wh), 2 * sizeof(int)));
+    // two ints of device scratch per device, allocated once per process (the call synchronises anyway, so
+    // concurrent callers are serialised by the lock)
+    static std::mutex lock;
+    static int *scratch[64] = {};
+    int dev = 0;
+    SYNIM_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(SYNIM_ERR_INVALID_ARG, "synim_bbox_extent: device index %d out of range", dev);
+    std::lock_guard<std::mutex> guard(lock);
+    if (!scratch[dev]) SYNIM_CUDA(cudaMalloc(reinterpret_cast<void **>(&scratch[dev]), 2 * sizeof(int)));
+    int *d_wh = scratch[dev];
     int wh[2] = {0, 0};
     cudaError_t e = synim::launch_bbox_extent(d_bbox, n_modes, d_wh, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(wh, d_wh, sizeof(wh), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    cudaFree(d_wh);
     if (e != cudaSuccess) return cuda_fail(e, "synim_bbox_extent");
     *max_w = wh[0]; *max_h = wh[1];
     return SYNIM_OK;
@@ -547,7 +562,10 @@ synim_status synim_interaction_matrix_host(const synim_geometry *g, const float 
         st = run_interaction_matrix(g, g->ws_cube, pny, pnx, g->ws_bbox + 4 * (size_t)n_modes, n_modes, g->ws_bbox, nullptr, bw, bh,
                                     affine, mode, g->ws_out, g->rows, s);
     }
-    if (st != SYNIM_OK) return st;
+    if (st != SYNIM_OK) {
+        cudaStreamSynchronize(s);   // the staging buffers may still be in flight: they are reused by the next call
+        return st;
+    }
     SYNIM_CUDA(cudaMemcpyAsync(h_out, g->ws_out, out_bytes, cudaMemcpyDeviceToHost, s));
     SYNIM_CUDA(cudaStreamSynchronize(s));
     return SYNIM_OK;

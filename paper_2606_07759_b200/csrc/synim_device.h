@@ -58,5 +58,7 @@ cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int 
                                   cudaStream_t stream);
 cudaError_t launch_bbox_extent(const int *d_bbox, int n_modes, int *d_wh, cudaStream_t stream);
 size_t max_dynamic_smem();  // opt-in limit of the current device (bytes)
+void note_launch();           // every launcher calls this once per kernel it enqueues (synim_launch_count)
+long long launches_so_far();
 
 }  // namespace synim

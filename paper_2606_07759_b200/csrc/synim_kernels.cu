@@ -3,6 +3,8 @@
 // (bounding boxes and diagonal extents).  The hot path (S1-S4) is synim_strip.cu.
 #include "synim_device.h"
 
+#include <atomic>
+
 namespace synim {
 
 namespace {
@@ -148,6 +150,10 @@ __global__ void __launch_bounds__(256) bbox_extent_kernel(const int *__restrict_
 
 }  // namespace
 
+static std::atomic<long long> g_launches{0};
+void note_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+long long launches_so_far() { return g_launches.load(std::memory_order_relaxed); }
+
 size_t max_dynamic_smem()
 {
     int dev = 0, v = 0;
@@ -159,6 +165,7 @@ size_t max_dynamic_smem()
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
                                  float *d_wmap, int *d_error_flag, cudaStream_t stream)
 {
+    note_launch();
     subap_weights_kernel<<<n_subap * n_subap, 128, 0, stream>>>(d_pupil, d_valid, n_subap, n_pix, d_wmap,
                                                                 d_error_flag);
     return cudaGetLastError();
@@ -167,6 +174,7 @@ cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, i
 cudaError_t launch_gtilt_maps(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix, float *d_gx, float *d_gy,
                               cudaStream_t stream)
 {
+    note_launch();
     gtilt_maps_kernel<<<n_subap * n_subap, 128, 0, stream>>>(d_pupil, d_valid, n_subap, n_pix, d_gx, d_gy);
     return cudaGetLastError();
 }
@@ -175,12 +183,14 @@ cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int 
                                   cudaStream_t stream)
 {
     if (n_modes <= 0) return cudaSuccess;
+    note_launch();
     bbox_kernel<<<n_modes, 256, 0, stream>>>(d_cube, ny, nx, d_bbox, d_diag);
     return cudaGetLastError();
 }
 
 cudaError_t launch_bbox_extent(const int *d_bbox, int n_modes, int *d_wh, cudaStream_t stream)
 {
+    note_launch();
     bbox_extent_kernel<<<1, 256, 0, stream>>>(d_bbox, n_modes, d_wh);
     return cudaGetLastError();
 }

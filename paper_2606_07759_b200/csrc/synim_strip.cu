@@ -659,6 +659,7 @@ cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_
     }
     CUtensorMap tm;
     memcpy(&tm, tensor_map, sizeof(tm));
+    note_launch();
     kernel<<<dim3((unsigned)p.n_modes, (unsigned)(p.chunks > 0 ? p.chunks : 1)), kStripThreads, smem_bytes, stream>>>(p, tm);
     return cudaGetLastError();
 }

@@ -22,7 +22,8 @@ SLOPES_ND, SLOPES_GTILT = 0, 1
 #: every symbol include/synim.h declares
 EXPORTS = ("synim_compose_affine", "synim_create_geometry", "synim_num_rows", "synim_num_valid",
            "synim_row_offset", "synim_interaction_matrix", "synim_compute_bboxes", "synim_bbox_extent",
-           "synim_interaction_matrix_host", "synim_destroy", "synim_last_error", "synim_version")
+           "synim_interaction_matrix_host", "synim_destroy", "synim_last_error", "synim_version",
+           "synim_launch_count")
 
 PHYSICAL_FIELDS = ("shift_x", "shift_y", "rot_deg", "mag_x", "mag_y",
                    "dm_shift_x", "dm_shift_y", "dm_rot_deg", "dm_mag",
@@ -86,6 +87,8 @@ def lib() -> ctypes.CDLL:
         L.synim_last_error.argtypes = []
         L.synim_version.restype = i32
         L.synim_version.argtypes = []
+        L.synim_launch_count.restype = i64
+        L.synim_launch_count.argtypes = []
         _lib = L
     return _lib
 
@@ -97,6 +100,16 @@ def _check(status: int) -> None:
 
 def version() -> int:
     return int(lib().synim_version())
+
+
+def launch_count() -> int:
+    """Kernels launched by the library in this process so far (synim_launch_count)."""
+    return int(lib().synim_launch_count())
+
+
+def hot_kernel_name(dense: bool) -> str:
+    """Name of the kernel that dominates a step (for reports; the launch lists under profiles/ show it)."""
+    return "synim_strip_kernel<false> (dense modes: source-space pieces)" if dense else "synim_strip_kernel<false>"
 
 
 def last_error() -> str:
@@ -259,10 +272,24 @@ def interaction_matrix_host(geom: Geometry, cube_host, bbox_host, affines: Seque
     def ptr(x):
         return x.data_ptr() if isinstance(x, torch.Tensor) else x.ctypes.data
 
+    def check(x, name, dtype_t, dtype_n, shape):
+        if isinstance(x, torch.Tensor):
+            ok = (not x.is_cuda) and x.dtype == dtype_t and x.is_contiguous()
+        else:
+            ok = isinstance(x, np.ndarray) and x.dtype == dtype_n and x.flags["C_CONTIGUOUS"]
+        if not ok or tuple(x.shape) != tuple(shape):
+            raise ValueError(f"{name} must be a C-contiguous host array of {dtype_n.__name__} with shape {tuple(shape)}")
+
     n = int(cube_host.shape[0])
     rows = geom.num_rows
+    check(cube_host, "cube_host", torch.float32, np.float32, (n, geom.ny, geom.nx))
+    if bbox_host is not None:
+        check(bbox_host, "bbox_host", torch.int32, np.int32, (n, 4))
+    if len(affines) != geom.n_wfs:
+        raise ValueError("one affine per sensor")
     if out_host is None:
         out_host = torch.empty((n, rows), dtype=torch.float32).pin_memory()
+    check(out_host, "out_host", torch.float32, np.float32, (n, rows))
     arr = _affine_array(affines, scales)
     _check(lib().synim_interaction_matrix_host(geom._h, ptr(cube_host), n,
                                                None if bbox_host is None else ptr(bbox_host),

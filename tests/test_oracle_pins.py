@@ -288,6 +288,66 @@ def test_gtilt_partial_subaperture_uses_first_and_last_valid_pixel():
     assert np.allclose(s[:4], 0.25, atol=1e-12) and np.allclose(s[4:], 0.0, atol=1e-12)
 
 
+def test_gtilt_threshold_and_aggregation_on_a_ragged_fractional_pupil():
+    """Pins the two decisions of reading R13 that a tilt or a full pupil cannot see (PAPER.md:61
+    "evaluates the phase difference strictly at the subaperture edges"):
+      * a pixel is valid iff P >= 0.5 (a pixel with 0 < P < 0.5 is NOT an edge; P == 0.5 is),
+      * the estimator is sum(num) / sum(den) over the pixel rows, not the mean of per-row ratios.
+    phi = x^2 (y^2) under the identity map is exact on integer pixels, so the closed form is
+    sum_rows(x_l^2 - x_f^2) / sum_rows(x_l - x_f) with (f, l) the first / last pixel of each row
+    with P >= 0.5.  Rows have different spans and the span ends are flanked by pixels of weight
+    0.3 / 0.49 (invalid) or exactly 0.5 (valid), so either mistake changes the value."""
+    n = 12
+    m = 2 * n
+    xs, ys = centred(m, m)
+    spans = [(2, 9), (1, 10), (3, 9), (0, 11), (4, 10), (2, 9), (4, 11), (1, 9), (3, 11), (0, 9), (1, 10), (2, 11)]
+    for axis in (0, 1):
+        pupil = np.zeros((m, m), np.float32)
+        expect = np.zeros((2, 2))
+        for a in range(2):
+            for b in range(2):
+                num = den = 0.0
+                ratios = []
+                for q, (f, l) in enumerate(spans):
+                    f, l = (f + a + b) % 5, l - ((a + 2 * b) % 3)           # a different ragged shape per subaperture
+                    line = np.zeros(n, np.float32)
+                    line[f:l + 1] = 1.0
+                    line[f] = 0.5                                           # exactly 0.5 counts as valid
+                    if f > 0:
+                        line[f - 1] = 0.3 if q % 2 else 0.49                # fractional, below the threshold
+                    if l + 1 < n:
+                        line[l + 1] = 0.3
+                    if axis == 0:
+                        pupil[a * n + q, b * n:(b + 1) * n] = line
+                        c = xs[0, b * n:(b + 1) * n]
+                    else:
+                        pupil[a * n:(a + 1) * n, b * n + q] = line
+                        c = ys[a * n:(a + 1) * n, 0]
+                    num += c[l] ** 2 - c[f] ** 2
+                    den += c[l] - c[f]
+                    ratios.append((c[l] ** 2 - c[f] ** 2) / (c[l] - c[f]))
+                expect[a, b] = num / den
+                assert abs(np.mean(ratios) - expect[a, b]) > 1e-2           # the aggregation is visible here
+        g = ((xs if axis == 0 else ys) ** 2).astype(np.float32)[None]
+        s = O.slopes_wfs(g, pupil, 2, n, np.ones((2, 2), np.uint8), IDENT, scale=1.0, mode=O.GTILT)[0]
+        got = s[:4] if axis == 0 else s[4:]
+        assert np.allclose(got.reshape(2, 2), expect, rtol=0, atol=1e-12), (axis, got, expect)
+        # the value with every lit pixel (P > 0) taken as valid is different: the threshold is visible too
+        lit = pupil > 0
+        alt = np.zeros((2, 2))
+        for a in range(2):
+            for b in range(2):
+                num = den = 0.0
+                for q in range(n):
+                    row = lit[a * n + q, b * n:(b + 1) * n] if axis == 0 else lit[a * n:(a + 1) * n, b * n + q]
+                    c = xs[0, b * n:(b + 1) * n] if axis == 0 else ys[a * n:(a + 1) * n, 0]
+                    k = np.flatnonzero(row)
+                    num += c[k[-1]] ** 2 - c[k[0]] ** 2
+                    den += c[k[-1]] - c[k[0]]
+                alt[a, b] = num / den
+        assert np.abs(alt - expect).min() > 1e-2
+
+
 # ---------------------------------------------------------------- composition helper
 def _sequential(phys, pt):
     """Apply the individual maps to a point one after another (independent restatement)."""

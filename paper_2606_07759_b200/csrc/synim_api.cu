@@ -48,6 +48,8 @@ struct WfsHost {
     float *d_wmap = nullptr;
     float *d_gx = nullptr, *d_gy = nullptr;   // G-tilt coefficient maps
     int *d_subap_row = nullptr;
+    int owner = -1;   // sensor that owns the four device maps (sensors with the same pupil, grid and valid mask
+                      // share one set: their lines then hit in L1 / L2 whichever sensor a warp works on)
 };
 
 }  // namespace
@@ -190,7 +192,9 @@ synim_status synim_compose_affine(const synim_wfs_physical *p, synim_wfs_affine 
 void synim_destroy(synim_geometry *g)
 {
     if (!g) return;
-    for (auto &w : g->wfs) {
+    for (size_t k = 0; k < g->wfs.size(); ++k) {
+        auto &w = g->wfs[k];
+        if (w.owner != (int)k) continue;   // shared maps are freed by their owner
         if (w.d_wmap) cudaFree(w.d_wmap);
         if (w.d_gx) cudaFree(w.d_gx);
         if (w.d_gy) cudaFree(w.d_gy);
@@ -248,6 +252,7 @@ synim_status synim_create_geometry(int32_t ny, int32_t nx, int32_t n_wfs, const 
     for (int w = 0; w < n_wfs; ++w) {
         WfsHost &h = g->wfs[w];
         h.n_subap = grids[w].n_subap; h.n_pix = grids[w].n_pix; h.M = h.n_subap * h.n_pix;
+        h.owner = w;
         const size_t ns = (size_t)h.n_subap * h.n_subap;
         rowmap.assign(ns, -1);
         valid01.assign(ns, 0);
@@ -255,9 +260,22 @@ synim_status synim_create_geometry(int32_t ny, int32_t nx, int32_t n_wfs, const 
         for (size_t q = 0; q < ns; ++q)
             if (grids[w].valid_mask[q]) { rowmap[q] = k++; valid01[q] = 1; }
         h.n_valid = k;
-        if (row + 2LL * k > 0x7fffffffLL) return cleanup(fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: more than 2^31 rows"));
+        if (row + 2LL * k > 0x3fffffffLL) return cleanup(fail(SYNIM_ERR_INVALID_ARG, "synim_create_geometry: more than 2^30 rows"));
         h.row_x = (int)row; h.row_y = (int)row + k;
         row += 2LL * k;
+        // the same pupil buffer, grid and valid mask as an earlier sensor: share its maps
+        for (int v = 0; v < w; ++v) {
+            if (g->wfs[v].owner != v || grids[v].d_pupil != grids[w].d_pupil || grids[v].n_subap != h.n_subap ||
+                grids[v].n_pix != h.n_pix)
+                continue;
+            bool same = true;
+            for (size_t q = 0; q < ns && same; ++q) same = (grids[v].valid_mask[q] != 0) == (valid01[q] != 0);
+            if (!same) continue;
+            h.owner = v;
+            h.d_wmap = g->wfs[v].d_wmap; h.d_gx = g->wfs[v].d_gx; h.d_gy = g->wfs[v].d_gy; h.d_subap_row = g->wfs[v].d_subap_row;
+            break;
+        }
+        if (h.owner != w) continue;
         // rows of zeros below the map: the strip kernel's halo lanes and row look-ahead read them
         const size_t wmap_bytes = sizeof(float) * (size_t)(h.M + synim::kWmapPadRows) * h.M;
         if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_wmap), wmap_bytes)) != cudaSuccess)
@@ -270,7 +288,7 @@ synim_status synim_create_geometry(int32_t ny, int32_t nx, int32_t n_wfs, const 
             return cleanup(cuda_fail(e, "cudaMemcpyAsync(subap_row)"));
         if ((e = cudaMemcpyAsync(d_valid, valid01.data(), ns, cudaMemcpyHostToDevice, s)) != cudaSuccess)
             return cleanup(cuda_fail(e, "cudaMemcpyAsync(valid)"));
-        if ((e = synim::launch_subap_weights(grids[w].d_pupil, d_valid, h.n_subap, h.n_pix, h.d_wmap, d_err, s)) != cudaSuccess)
+        if ((e = synim::launch_subap_weights(grids[w].d_pupil, d_valid, h.n_subap, h.n_pix, h.d_wmap, h.d_subap_row, d_err, s)) != cudaSuccess)
             return cleanup(cuda_fail(e, "subap_weights_kernel"));
         // the G-tilt estimator's coefficient maps, same layout
         if ((e = cudaMalloc(reinterpret_cast<void **>(&h.d_gx), wmap_bytes)) != cudaSuccess) return cleanup(cuda_fail(e, "cudaMalloc(gx)"));
@@ -363,14 +381,27 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         d.scale = (float)affine[w].slope_scale;
         d.M = h.M; d.n_subap = h.n_subap; d.n_pix = h.n_pix; d.row_x = h.row_x; d.row_y = h.row_y;
         d.tab_off = 0; d.tab_cap = 0;
+        d.w_uniform = (float)(0.5 / ((double)h.n_pix * (double)h.n_pix));
+        d.spb = h.n_pix <= synim::kStripMaxCols ? synim::kStripMaxCols / h.n_pix : 0;
+        d.red_steps = 0;
+        while (d.red_steps < 5 && (1 << d.red_steps) < h.n_pix) ++d.red_steps;
         d.npx_magic = (unsigned)((0x100000000ULL + (unsigned long long)h.n_pix - 1) / (unsigned long long)h.n_pix);   // (unused for 1)
+    }
+    // launch groups: consecutive sensors of one class (subapertures that fit a strip / giant ones), at most
+    // kMaxWfsPerLaunch each; a group's rows are contiguous in the column
+    std::vector<std::pair<int, int>> groups;   // [first, last) sensor
+    for (int w = 0; w < n_wfs;) {
+        int e = w + 1;
+        while (e < n_wfs && e - w < synim::kMaxWfsPerLaunch && (dev[e].spb > 0) == (dev[w].spb > 0)) ++e;
+        groups.emplace_back(w, e);
+        w = e;
     }
     // per sensor a table of (x, y) partial slopes over the window of subapertures one piece's footprint
     // can span (the kernel derives the window from the same bounds and traps if it ever needed more)
     int tab_floats_max = 0;
-    for (int w0 = 0; w0 < n_wfs; w0 += synim::kMaxWfsPerLaunch) {
+    for (const auto &gr : groups) {
         int off = 0;
-        for (int w = w0; w < std::min(n_wfs, w0 + synim::kMaxWfsPerLaunch); ++w) {
+        for (int w = gr.first; w < gr.second; ++w) {
             synim::WfsDev &d = dev[w];
             const double ej = (cap_w + 2) * std::fabs(d.inv[0]) + (cap_h + 2) * std::fabs(d.inv[1]);
             const double ei = (cap_w + 2) * std::fabs(d.inv[3]) + (cap_h + 2) * std::fabs(d.inv[4]);
@@ -403,8 +434,8 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         if (ld == g->rows) SYNIM_CUDA(cudaMemsetAsync(d_out, 0, sizeof(float) * (size_t)g->rows * n_modes, s));
         else SYNIM_CUDA(cudaMemset2DAsync(d_out, sizeof(float) * (size_t)ld, 0, sizeof(float) * (size_t)g->rows, n_modes, s));
     }
-    for (int w0 = 0; w0 < n_wfs; w0 += synim::kMaxWfsPerLaunch) {
-        const int nw = std::min(synim::kMaxWfsPerLaunch, n_wfs - w0);
+    for (const auto &gr : groups) {
+        const int w0 = gr.first, nw = gr.second - gr.first;
         synim::ImParams p;
         std::memset(&p, 0, sizeof(p));
         p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.origin = d_origin; p.out = d_out; p.ld = ld;

@@ -8,6 +8,9 @@ namespace synim {
 
 constexpr int kMaxWfsPerLaunch = 16;   // per-launch WFS batch (kernel-parameter space is 4 KB)
 constexpr int kWmapPadRows = 8;        // rows of zeros below each sensor's weight map (the kernel's look-ahead)
+constexpr int kSubapGeneral = 1 << 30; // flag in a row-map entry: valid subaperture whose pixel weights differ
+constexpr int kSubapRowMask = kSubapGeneral - 1;
+constexpr int kStripMaxCols = 30;      // D columns of a strip (one per lane, plus a halo lane on either side)
 
 // One sensor as the kernel sees it.  All coordinates are ABSOLUTE pixel indices: WFS pixel (i, j)
 // (row, column) samples the source grid at
@@ -20,9 +23,14 @@ struct WfsDev {
     double inv[6];
     const float *wmap;       // [M][M]  0.5*P/W_S, 0 where the subaperture is invalid
     const float *gx, *gy;    // [M][M]  G-tilt coefficients (gtilt_maps_kernel); same rows of zeros below
-    const int *subap_row;    // [n_subap^2] index among the valid subapertures, -1 if invalid
+    const int *subap_row;    // [n_subap^2] index among the valid subapertures (| kSubapGeneral if its pixel weights
+                             // differ), -1 if invalid
     float scale;             // slope_scale
+    float w_uniform;         // 0.5 / n_pix^2: the weight of every pixel of a uniform subaperture
     int M, n_subap, n_pix;
+    int spb;                 // subapertures per strip when strips are aligned to subaperture columns
+                             // (floor(30 / n_pix)); 0: subapertures wider than a strip, unaligned strips
+    int red_steps;           // ceil(log2(n_pix)) capped at 5: shuffle steps of the segmented lane reduction
     unsigned npx_magic;      // ceil(2^32 / n_pix): x / n_pix = umulhi(x, npx_magic) for the pixel indices met here
     int row_x, row_y;        // first row of the x / y slopes of this sensor inside a column
     int tab_off, tab_cap;    // this sensor's slice of the CTA's slope table (floats)
@@ -51,7 +59,7 @@ struct ImParams {
 // {patch_pitch, patch_h, 1}
 cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
-                                 float *d_wmap, int *d_error_flag, cudaStream_t stream);
+                                 float *d_wmap, int *d_subap_row, int *d_error_flag, cudaStream_t stream);
 cudaError_t launch_gtilt_maps(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix, float *d_gx, float *d_gy,
                               cudaStream_t stream);
 cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int nx, int *d_bbox, int *d_diag,

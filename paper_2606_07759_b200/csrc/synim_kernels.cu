@@ -10,26 +10,41 @@ namespace synim {
 namespace {
 
 // ---- geometry-time kernels ----------------------------------------------------------------------
-// one CTA per subaperture: W_S = sum of P, then wmap = 0.5*P/W_S (0 if invalid)
+// one CTA per subaperture: W_S = sum of P, then wmap = 0.5*P/W_S (0 if invalid).  A valid subaperture whose
+// n_pix^2 weights are not all equal gets kSubapGeneral set in its row-map entry: the others ("uniform":
+// fully and evenly lit, the common case under a binary pupil) have the constant weight 0.5/n_pix^2, which the
+// strip kernel applies once per subaperture to edge sums instead of once per pixel (synim_strip.cu).
 __global__ void __launch_bounds__(128) subap_weights_kernel(const float *__restrict__ pupil,
                                                             const uint8_t *__restrict__ valid, int n_subap,
-                                                            int n_pix, float *__restrict__ wmap, int *err)
+                                                            int n_pix, float *__restrict__ wmap, int *__restrict__ subap_row,
+                                                            int *err)
 {
     __shared__ double part[4];
+    __shared__ float pmin[4], pmax[4];
     __shared__ double total;
     const int s = blockIdx.x, a = s / n_subap, b = s - a * n_subap;
     const int M = n_subap * n_pix, n = n_pix * n_pix;
     double acc = 0.0;
+    float lo = 3.0e38f, hi = -3.0e38f;
     for (int e = threadIdx.x; e < n; e += 128) {
         const int r = e / n_pix, c = e - r * n_pix;
-        acc += (double)pupil[(size_t)(a * n_pix + r) * M + b * n_pix + c];
+        const float pv = pupil[(size_t)(a * n_pix + r) * M + b * n_pix + c];
+        acc += (double)pv;
+        lo = fminf(lo, pv); hi = fmaxf(hi, pv);
     }
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    for (int o = 16; o > 0; o >>= 1) {
+        acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if ((threadIdx.x & 31) == 0) { part[threadIdx.x >> 5] = acc; pmin[threadIdx.x >> 5] = lo; pmax[threadIdx.x >> 5] = hi; }
     __syncthreads();
     if (threadIdx.x == 0) {
         total = part[0] + part[1] + part[2] + part[3];
         if (valid[s] && !(total > 0.0)) atomicExch(err, 1);
+        const float l = fminf(fminf(pmin[0], pmin[1]), fminf(pmin[2], pmin[3]));
+        const float h = fmaxf(fmaxf(pmax[0], pmax[1]), fmaxf(pmax[2], pmax[3]));
+        if (valid[s] && !(l == h)) subap_row[s] |= kSubapGeneral;   // (the host wrote the row index, >= 0, before this launch)
     }
     __syncthreads();
     const bool ok = valid[s] && total > 0.0;
@@ -163,10 +178,10 @@ size_t max_dynamic_smem()
 }
 
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
-                                 float *d_wmap, int *d_error_flag, cudaStream_t stream)
+                                 float *d_wmap, int *d_subap_row, int *d_error_flag, cudaStream_t stream)
 {
     note_launch();
-    subap_weights_kernel<<<n_subap * n_subap, 128, 0, stream>>>(d_pupil, d_valid, n_subap, n_pix, d_wmap,
+    subap_weights_kernel<<<n_subap * n_subap, 128, 0, stream>>>(d_pupil, d_valid, n_subap, n_pix, d_wmap, d_subap_row,
                                                                 d_error_flag);
     return cudaGetLastError();
 }

@@ -52,7 +52,7 @@ constexpr int kStripThreads = kComputeThreads;
 constexpr int kStripUnroll = SYNIM_STRIP_UNROLL;
 constexpr int kStripRows = SYNIM_STRIP_ROWS;
 static_assert(2 * kStripRows <= kWmapPadRows, "weight look-ahead runs past the rows of zeros");
-constexpr int kStripCols = 30;               // D columns per strip: lanes 1..30, halo on lanes 0 and 31
+constexpr int kStripCols = kStripMaxCols;     // D columns per strip: lanes 1..30, halo on lanes 0 and 31
 constexpr float kMagicFloor = 12582912.0f;   // 1.5 * 2^23: fadd.rm(x, magic) = magic + floor(x), |x| < 2^22
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -194,15 +194,32 @@ __device__ __forceinline__ float wld(const float *p)
 __device__ __forceinline__ int div_npx(int x, int npx, unsigned magic) { return npx == 1 ? x : (int)__umulhi((unsigned)x, magic); }
 
 // One strip: D columns jA .. jA+nC-1 (lanes 1..nC), D rows i0 .. i1 of sensor W.
-// Its partial slopes are added to the CTA's shared table: entry (a, b, axis) of the sensor's window of
+// Its partial slopes go to the CTA's shared table: entry (a, b, axis) of the sensor's window of
 // subapertures (first row a0, first column b0, nb columns) sits at tab + ((a-a0)*nb + (b-b0))*8 + axis*4.
+//
+// kAligned (the sensor's subapertures are at most a strip wide): the strip starts on a subaperture boundary
+// and holds whole subaperture columns only, so (a) each table entry is written by exactly one warp, with a
+// plain store, and (b) the rows of the strip are cut into SEGMENTS of consecutive "units" (the strip's
+// subapertures of one subaperture row) of one kind.  A unit none of whose valid subapertures has unequal
+// pixel weights (the row map flags those with kSubapGeneral at geometry time) is an EDGE-SUM unit: with a
+// constant weight w = 0.5/n^2 the weighted sum of central differences telescopes,
+//     sum_S w*D_x = w * sum_rows (phi[.,j0+n] + phi[.,j0+n-1] - phi[.,j0] - phi[.,j0-1]),
+//     sum_S w*D_y = w * sum_cols (phi[i0+n,.] + phi[i0+n-1,.] - phi[i0,.] - phi[i0-1,.]),
+// (the identity behind tests/test_oracle_pins.py::test_telescoping_identity_on_full_subapertures), so a pixel
+// row costs its sample and ONE add: no stencil shuffles, no weight loads, no multiply; the lanes are combined
+// once per subaperture.  The other units (a partially lit subaperture among them) take the general path:
+// D_y from registers, D_x from the neighbouring lanes, one weight per pixel.  Each segment primes its own
+// two rows of phi, so the two loops share no state but the table.
 // kGtilt: the G-tilt estimator (reading R13) instead of the numerical derivative: the slopes are then two
 // weighted sums of phi itself (coefficient maps gx, gy: +-1/den on the first / last valid pixel of every
-// pixel row / column of a subaperture), so the stencil and its shuffles drop out.
-template <bool kGtilt>
+// pixel row / column of a subaperture), so the stencil and its shuffles drop out (general path only).
+template <bool kGtilt, bool kAligned>
 __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
                                               uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp)
 {
+    constexpr bool kEdge = kAligned && !kGtilt;   // the edge-sum path exists
+    constexpr int kRows = kStripRows;
+    static_assert(kRows == 2, "the segment loops are written for two rows per iteration");
     const int lane = threadIdx.x & 31;
     const int nR = i1 - i0 + 1;   // D rows; phi row rr (0 .. nR+1) is absolute row i0-1+rr
     const int jcol = jA - 1 + lane;
@@ -239,12 +256,8 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     const int d_lo = max(first - 1, 1), d_hi = min(last + 1, nR);   // D rows that can be non-zero
     if (d_hi < d_lo) return;
 
-    StripSensor S;
-    S.wmap = kGtilt ? W.gx : W.wmap; S.wmap2 = kGtilt ? W.gy : W.wmap;
-    S.M = W.M; S.n_subap = W.n_subap; S.n_pix = W.n_pix;
-
     // segments of lanes that belong to one subaperture column
-    const int npx = S.n_pix;
+    const int npx = W.n_pix, n_subap = W.n_subap;
     const bool isD = lane >= 1 && lane <= nC;
     const int seg = isD ? div_npx(jcol, npx, W.npx_magic) : -1;
     const int segL = __shfl_up_sync(kFull, seg, 1);
@@ -255,36 +268,76 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         const int sd = __shfl_down_sync(kFull, seg, 1 << s);
         if (isD && lane + (1 << s) < 32 && sd == seg) okm |= 1u << s;
     }
+    const int nsteps = kAligned ? W.red_steps : 5;   // (warp-uniform) a lane segment is at most n_pix lanes long
 
     const int i_first = i0 - 1 + d_lo;           // absolute row of D row d_lo
-    int a_cur = div_npx(i_first, npx, W.npx_magic);
+    const int a_first = div_npx(i_first, npx, W.npx_magic);
+    int a_cur = a_first;
     int rem = i_first - a_cur * npx;             // rows of subaperture row a_cur already behind us
-    const int M = S.M;
-    // weight map offsets (elements).  The map has kWmapPadRows rows of zeros below row M-1: halo lanes stay
-    // on the first of them (stride 0), and the look-ahead of the last rows may run onto them.
-    uint32_t woff = isD ? (uint32_t)i_first * (uint32_t)M + (uint32_t)jcol : (uint32_t)M * (uint32_t)M;
-    const uint32_t wrow = isD ? (uint32_t)M : 0u, wstride = isD ? (uint32_t)kStripRows * (uint32_t)M : 0u;
+    const int M = W.M;
     uint32_t tent = tab + (uint32_t)((a_cur - a0) * nb + (isD ? seg - b0 : 0)) * 8u;   // this lane's table entry
     const uint32_t tstep = (uint32_t)nb * 8u;
 
-    // S3 (columns): segmented sum over the lanes of a subaperture, then one shared-memory add per axis
-    auto flush = [&](float sx, float sy) {
+    // bit u of genmask: unit a_first+u needs the general path (lane u looks at the strip's subapertures of
+    // its unit; units beyond 32 are simply taken as general)
+    unsigned genmask = 0xffffffffu;
+    if (kEdge) {
+        const int bA = div_npx(jA, npx, W.npx_magic), nsb = div_npx(nC, npx, W.npx_magic);
+        const int a_mine = a_first + lane;
+        bool gflag = false;
+        if (a_mine < n_subap) {
+            const int *rp = W.subap_row + a_mine * n_subap + bA;
+            for (int q = 0; q < nsb; ++q)
+                if (bA + q < n_subap) { const int c = __ldg(rp + q); gflag = gflag || (c >= 0 && (c & kSubapGeneral) != 0); }
+        }
+        genmask = __ballot_sync(kFull, gflag);
+    }
+
+    // S3 (columns), general path: segmented sum over the lanes of a subaperture, then one shared-memory
+    // store (this warp owns the entry) or add (another warp may hold the other columns of this subaperture)
+    auto flush_general = [&](float sx, float sy) {
         unsigned m = okm;
         asm volatile("" : "+r"(m));   // keeps the five lane masks out of predicate registers between flushes
 #pragma unroll
         for (int s = 0; s < 5; ++s) {   // (a step beyond the segment length has no lane mask set: cheaper than a branch)
+            if (kAligned && s >= nsteps) break;
             const float tx = __shfl_down_sync(kFull, sx, 1 << s), ty = __shfl_down_sync(kFull, sy, 1 << s);
             if ((m >> s) & 1u) { sx += tx; sy += ty; }
         }
-        if (head && (sx != 0.0f || sy != 0.0f) && a_cur < S.n_subap) {
+        if (head && (kAligned || sx != 0.0f || sy != 0.0f) && a_cur < n_subap) {
 #ifdef SYNIM_CHECKS
             if (tent < tab || tent + 8u > tab + (uint32_t)W.tab_cap * 4u) __trap();
 #endif
-            red_shared_f32(tent, sx);   // another warp may hold the other columns of this subaperture
-            red_shared_f32(tent + 4u, sy);
+            if (kAligned) {
+                sts_f32(tent, sx);
+                sts_f32(tent + 4u, sy);
+            } else {
+                red_shared_f32(tent, sx);
+                red_shared_f32(tent + 4u, sy);
+            }
         }
-        ++a_cur;
-        tent += tstep;
+    };
+    // edge-sum path: cs = this lane's column sum of phi over the unit's rows, v = (phi[i0+n] + phi[i0+n-1]) -
+    // (phi[i0] + phi[i0-1]) of this lane's column
+    const float wu = W.w_uniform;
+    auto flush_edges = [&](float cs, float v) {
+        const float pr = cs + __shfl_up_sync(kFull, cs, 1);                  // columns j-1 and j
+        const float sx = (__shfl_down_sync(kFull, pr, npx) - pr) * wu;       // at the head lane: the two edge pairs
+        unsigned m = okm;
+        asm volatile("" : "+r"(m));
+#pragma unroll
+        for (int s = 0; s < 5; ++s) {
+            if (s >= nsteps) break;
+            const float t = __shfl_down_sync(kFull, v, 1 << s);
+            if ((m >> s) & 1u) v += t;
+        }
+        if (head && a_cur < n_subap) {
+#ifdef SYNIM_CHECKS
+            if (tent < tab || tent + 8u > tab + (uint32_t)W.tab_cap * 4u) __trap();
+#endif
+            sts_f32(tent, sx);
+            sts_f32(tent + 4u, v * wu);
+        }
     };
 
     // S2: one bilinear sample of phi row rf from the staged pixels; 0 outside them.  Non-negative floats order like
@@ -330,69 +383,107 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
               "r"(rpitch4));
         return phi;
     };
-
-    constexpr int kRows = kStripRows;
-    float rf = (float)(d_lo + 1);
-    float pmA = sample((float)(d_lo - 1)), pmB = sample((float)d_lo);   // phi[d-1], phi[d]
 #ifdef SYNIM_CHECKS
     const uint32_t wlimit = (uint32_t)(M + kWmapPadRows) * (uint32_t)M;
 #define SYNIM_WCHECK(o) do { if ((o) >= wlimit) __trap(); } while (0)
 #else
 #define SYNIM_WCHECK(o) do { } while (0)
 #endif
-    float wgt[kRows], wg2[kRows];
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-        SYNIM_WCHECK(woff + (uint32_t)k * wrow);
-        wgt[k] = wld(S.wmap + (woff + (uint32_t)k * wrow));
-        wg2[k] = kGtilt ? wld(S.wmap2 + (woff + (uint32_t)k * wrow)) : wgt[k];
-    }
-    float sx = 0.0f, sy = 0.0f;
-#pragma unroll(kStripUnroll)
-    for (int d = d_lo; d <= d_hi; d += kRows) {
-#pragma unroll
-        for (int q = 0; q < (kComputeWarps >= 4 ? 1 : 4 / kComputeWarps); ++q) zp.step();
-        float cur[kRows];   // phi[d+1 .. d+kRows]
-#pragma unroll
-        for (int k = 0; k < kRows; ++k) cur[k] = sample(rf + (float)k);
-        rf += (float)kRows;
-        // S3: D rows d .. d+kRows-1: D_y from registers, D_x from the neighbouring lanes.  A row past d_hi
-        // has D = 0 exactly (or a weight from the rows of zeros), so it needs no test.
-        float dx[kRows], dy[kRows];
-#pragma unroll
-        for (int k = 0; k < kRows; ++k) {
-            const float mid = k == 0 ? pmB : cur[k - 1];                         // phi[d+k]
-            const float above = k == 0 ? pmA : (k == 1 ? pmB : cur[k - 2]);     // phi[d+k-1]
-            if (kGtilt) {
-                dx[k] = mid; dy[k] = mid;   // the sums run over phi itself
-            } else {
-                dy[k] = cur[k] - above;
-                dx[k] = __shfl_down_sync(kFull, mid, 1) - __shfl_up_sync(kFull, mid, 1);
-            }
+
+    int d = d_lo;
+    while (d <= d_hi) {
+        // the segment: units of one kind from the current one on; D rows d .. d_end
+        const int u = a_cur - a_first;
+        const bool gen = !kEdge || u >= 32 || ((genmask >> u) & 1u);
+        int d_end = d_hi;
+        if (kEdge && u < 32) {
+            const unsigned other = (gen ? ~genmask : genmask) >> u;   // bit k: unit u+k is of the other kind
+            if (other) d_end = min(d_hi, (a_cur + __ffs(other) - 1) * npx - i0);   // last D row before that unit
         }
-        if (rem + kRows < npx) {   // warp-uniform: no subaperture row ends inside these rows
-#pragma unroll
-            for (int k = 0; k < kRows; ++k) { sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wg2[k], dy[k], sy); }
-            rem += kRows;
-        } else {
+        float rf = (float)(d + 1);
+        float pmA = sample((float)(d - 1)), pmB = sample((float)d);   // phi[d-1], phi[d]
+        if (gen) {
+            const float *wm = kGtilt ? W.gx : W.wmap, *wm2 = kGtilt ? W.gy : W.wmap;
+            // weight map offsets (elements).  The map has kWmapPadRows rows of zeros below row M-1: halo lanes
+            // stay on the first of them (stride 0), and the look-ahead of the last rows may run onto them.
+            uint32_t woff = isD ? (uint32_t)(i0 - 1 + d) * (uint32_t)M + (uint32_t)jcol : (uint32_t)M * (uint32_t)M;
+            const uint32_t wrow = isD ? (uint32_t)M : 0u, wstride = isD ? (uint32_t)kRows * (uint32_t)M : 0u;
+            float wgt[kRows], wg2[kRows];
 #pragma unroll
             for (int k = 0; k < kRows; ++k) {
-                sx = fmaf(wgt[k], dx[k], sx); sy = fmaf(wg2[k], dy[k], sy);
-                if (++rem == npx) { flush(sx, sy); sx = 0.0f; sy = 0.0f; rem = 0; }
+                SYNIM_WCHECK(woff + (uint32_t)k * wrow);
+                wgt[k] = wld(wm + (woff + (uint32_t)k * wrow));
+                wg2[k] = kGtilt ? wld(wm2 + (woff + (uint32_t)k * wrow)) : wgt[k];
             }
-        }
-        pmA = cur[kRows - 2]; pmB = cur[kRows - 1];
-        // the weights of the next kRows rows, loaded into the registers just consumed: nothing touches them
-        // until the end of the next iteration (a register-to-register copy would wait for the load)
-        woff += wstride;
+            float sx = 0.0f, sy = 0.0f;
+#pragma unroll(kStripUnroll)
+            for (; d <= d_end; d += kRows) {
 #pragma unroll
-        for (int k = 0; k < kRows; ++k) {
-            SYNIM_WCHECK(woff + (uint32_t)k * wrow);
-            wgt[k] = wld(S.wmap + (woff + (uint32_t)k * wrow));
-            wg2[k] = kGtilt ? wld(S.wmap2 + (woff + (uint32_t)k * wrow)) : wgt[k];
+                for (int q = 0; q < (kComputeWarps >= 4 ? 1 : 4 / kComputeWarps); ++q) zp.step();
+                float cur[kRows];   // phi[d+1 .. d+kRows]
+#pragma unroll
+                for (int k = 0; k < kRows; ++k) cur[k] = sample(rf + (float)k);
+                rf += (float)kRows;
+                // D rows d, d+1: D_y from registers, D_x from the neighbouring lanes.  A row past d_hi has D = 0
+                // exactly (or a weight from the rows of zeros); a row past d_end is the next segment's.
+                const bool two = !kEdge || d + 1 <= d_end;
+#pragma unroll
+                for (int k = 0; k < kRows; ++k) {
+                    const float mid = k == 0 ? pmB : cur[k - 1];                         // phi[d+k]
+                    const float above = k == 0 ? pmA : (k == 1 ? pmB : cur[k - 2]);     // phi[d+k-1]
+                    float dx, dy;
+                    if (kGtilt) {
+                        dx = mid; dy = mid;   // the sums run over phi itself
+                    } else {
+                        dy = cur[k] - above;
+                        dx = __shfl_down_sync(kFull, mid, 1) - __shfl_up_sync(kFull, mid, 1);
+                    }
+                    if (k == 0 || two) {
+                        sx = fmaf(wgt[k], dx, sx); sy = fmaf(wg2[k], dy, sy);
+                        if (++rem == npx) { flush_general(sx, sy); sx = 0.0f; sy = 0.0f; rem = 0; ++a_cur; tent += tstep; }
+                    }
+                }
+                pmA = cur[kRows - 2]; pmB = cur[kRows - 1];
+                // the weights of the next kRows rows, loaded into the registers just consumed: nothing touches
+                // them until the end of the next iteration (a register-to-register copy would wait for the load)
+                woff += wstride;
+#pragma unroll
+                for (int k = 0; k < kRows; ++k) {
+                    SYNIM_WCHECK(woff + (uint32_t)k * wrow);
+                    wgt[k] = wld(wm + (woff + (uint32_t)k * wrow));
+                    wg2[k] = kGtilt ? wld(wm2 + (woff + (uint32_t)k * wrow)) : wgt[k];
+                }
+            }
+            if (rem > 0 && d_end == d_hi) { flush_general(sx, sy); rem = 0; }   // the walk ended inside a unit
+        } else {
+            float cs = 0.0f;   // sum of phi over the rows of the unit so far
+            // phi[i0-1] + phi[i0] of the current unit: both rows lie above the walk (where phi is 0) unless the
+            // segment starts on the unit's first row
+            float utop = rem == 0 ? pmA + pmB : 0.0f;
+            for (; d <= d_end; d += kRows) {
+                zp.step();
+                const float c0 = sample(rf), c1 = sample(rf + 1.0f);   // phi[d+1], phi[d+2]
+                rf += 2.0f;
+                cs += pmB;                                            // D row d: phi[d]
+                if (++rem == npx) {   // the unit's last row: phi[i0+n-1] = phi[d], phi[i0+n] = phi[d+1]
+                    const float ubot = pmB + c0;
+                    flush_edges(cs, ubot - utop);
+                    utop = ubot; cs = 0.0f; rem = 0; ++a_cur; tent += tstep;
+                }
+                if (d + 1 <= d_end) {                                 // D row d+1 (else it is the next segment's)
+                    cs += c0;
+                    if (++rem == npx) {
+                        const float ubot = c0 + c1;
+                        flush_edges(cs, ubot - utop);
+                        utop = ubot; cs = 0.0f; rem = 0; ++a_cur; tent += tstep;
+                    }
+                }
+                pmA = c0; pmB = c1;
+            }
+            if (rem > 0 && d_end == d_hi) { flush_edges(cs, 0.0f - utop); rem = 0; }   // rows below the walk hold phi = 0
         }
+        d = d_end + 1;
     }
-    if (rem > 0) flush(sx, sy);
 }
 
 
@@ -442,17 +533,21 @@ __device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, 
 // All warps, after a barrier: fetch the IM rows of the windows' subapertures (needed only when the table
 // is stored: asynchronously, so that the store at the end waits for nothing), then sample the strips of
 // every sensor's footprint.
-template <bool kGtilt>
+template <bool kGtilt, bool kAligned>
 __device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, int lane, const int4 *s_box, const int4 *s_win,
                                                   int *s_next_ptr, const CellBox &cb, uint32_t tab_base, uint32_t krow_base,
                                                   ZeroPacer &zp)
 {
-    int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_nb = 0;
+    // kAligned (every sensor of the launch has subapertures that fit a strip, spb > 0): strip t holds the spb
+    // subaperture columns b0 + t*spb ... of the footprint's window; otherwise (giant subapertures) strips are
+    // kStripCols columns of the footprint, wherever they fall.  (The host never mixes the two in one launch.)
+    int r_i0 = 0, r_i1 = -1, r_j0 = 0, r_j1 = -1, r_n = 0, r_a0 = 0, r_b0 = 0, r_nb = 0, r_spb = 0;
     if (lane < p.n_wfs) {
         const int4 fb = s_box[lane], fw = s_win[lane];
         r_i0 = fb.x; r_i1 = fb.y; r_j0 = fb.z; r_j1 = fb.w;
         r_a0 = fw.x; r_b0 = fw.y; r_nb = fw.w;
-        if (r_j1 >= r_j0 && r_i1 >= r_i0) r_n = (r_j1 - r_j0 + kStripCols) / kStripCols;
+        r_spb = p.wfs[lane].spb;
+        if (r_j1 >= r_j0 && r_i1 >= r_i0) r_n = kAligned ? (r_nb + r_spb - 1) / r_spb : (r_j1 - r_j0 + kStripCols) / kStripCols;
     }
     // the IM rows of the windows' subapertures, needed only when the table is stored: fetched now,
     // asynchronously, so that the store at the end waits for nothing (sensor w by warp w mod 4)
@@ -485,9 +580,16 @@ __device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, i
         const int i0 = __shfl_sync(kFull, r_i0, w), i1 = __shfl_sync(kFull, r_i1, w);
         const int j0 = __shfl_sync(kFull, r_j0, w), j1 = __shfl_sync(kFull, r_j1, w);
         const int a0 = __shfl_sync(kFull, r_a0, w), b0 = __shfl_sync(kFull, r_b0, w), nb = __shfl_sync(kFull, r_nb, w);
-        const int jA = j0 + (t - base) * kStripCols;
-        const int nC = min(kStripCols, j1 - jA + 1);
-        process_strip<kGtilt>(p.wfs[w], i0, i1, jA, nC, cb, p.addr_bias, tab_base + (uint32_t)p.wfs[w].tab_off * 4u, a0, b0, nb, zp);
+        const int spb = __shfl_sync(kFull, r_spb, w);
+        const WfsDev &W = p.wfs[w];
+        const uint32_t tab = tab_base + (uint32_t)W.tab_off * 4u;
+        if (kAligned) {
+            const int bA = b0 + (t - base) * spb;
+            process_strip<kGtilt, true>(W, i0, i1, bA * W.n_pix, min(spb, b0 + nb - bA) * W.n_pix, cb, p.addr_bias, tab, a0, b0, nb, zp);
+        } else {
+            const int jA = j0 + (t - base) * kStripCols;
+            process_strip<kGtilt, false>(W, i0, i1, jA, min(kStripCols, j1 - jA + 1), cb, p.addr_bias, tab, a0, b0, nb, zp);
+        }
     }
 }
 
@@ -509,7 +611,7 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
             const int k = lds_s32(krow_base + (uint32_t)((W.tab_off >> 1) + (e >> 1)) * 4u);   // fetched while the strips ran
             if (kAtomic) sts_f32(tb + (uint32_t)e * 4u, 0.0f);
             if (k < 0) continue;
-            float *dst = colp + ((e & 1) ? W.row_y : W.row_x) + k;
+            float *dst = colp + ((e & 1) ? W.row_y : W.row_x) + (k & kSubapRowMask);
             if (kAtomic) {
                 atomicAdd(dst, v * W.scale);
             } else {
@@ -519,7 +621,7 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
     }
 }
 
-template <bool kGtilt>
+template <bool kGtilt, bool kAligned>
 __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
                                                                                      const __grid_constant__ CUtensorMap tmap)
 {
@@ -618,7 +720,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             }
             bar_sync(1, kComputeThreads);   // footprints (and a cleared ring) visible
 
-            sample_footprints<kGtilt>(p, warp, lane, s_box, s_win, &s_next, cb, tab_base, krow_base, zp);
+            sample_footprints<kGtilt, kAligned>(p, warp, lane, s_box, s_win, &s_next, cb, tab_base, krow_base, zp);
             if (multi) {
                 cp_async_wait_all();
                 bar_sync(1, kComputeThreads);   // every warp is done with this box and this piece's table
@@ -645,13 +747,18 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
 cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream)
 {
     if (p.n_modes <= 0) return cudaSuccess;
-    auto kernel = gtilt ? synim_strip_kernel<true> : synim_strip_kernel<false>;
+    bool aligned = true;   // one class of sensors per launch (the host groups them)
+    for (int w = 0; w < p.n_wfs; ++w) aligned = aligned && p.wfs[w].spb > 0;
+    for (int w = 0; w < p.n_wfs; ++w)
+        if (!aligned && p.wfs[w].spb > 0) return cudaErrorInvalidValue;
+    auto kernel = gtilt ? (aligned ? synim_strip_kernel<true, true> : synim_strip_kernel<true, false>)
+                        : (aligned ? synim_strip_kernel<false, true> : synim_strip_kernel<false, false>);
     // the opt-in shared-memory limit only ever has to grow (per device; a race sets it twice, harmlessly)
-    static size_t granted[2][64] = {};
+    static size_t granted[4][64] = {};
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    size_t &have = granted[gtilt ? 1 : 0][dev & 63];
+    size_t &have = granted[(gtilt ? 2 : 0) + (aligned ? 1 : 0)][dev & 63];
     if (smem_bytes > have) {
         e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return e;

@@ -151,12 +151,16 @@ class Geometry:
         n = len(wfs)
         grids = (WfsGrid * n)()
         keep = []
+        on_device = {}   # sensors that pass the SAME pupil object get the same device buffer (the library then shares their maps)
         for k, w in enumerate(wfs):
             valid = np.ascontiguousarray(w.valid, dtype=np.uint8)
-            pupil = w.pupil
-            if not isinstance(pupil, torch.Tensor):
-                pupil = torch.from_numpy(np.ascontiguousarray(pupil, dtype=np.float32))
-            pupil = pupil.to(device="cuda", dtype=torch.float32).contiguous()
+            pupil = on_device.get(id(w.pupil))
+            if pupil is None:
+                pupil = w.pupil
+                if not isinstance(pupil, torch.Tensor):
+                    pupil = torch.from_numpy(np.ascontiguousarray(pupil, dtype=np.float32))
+                pupil = pupil.to(device="cuda", dtype=torch.float32).contiguous()
+                on_device[id(w.pupil)] = pupil
             m = int(w.n_subap) * int(w.n_pix)
             if tuple(pupil.shape) != (m, m) or valid.shape != (w.n_subap, w.n_subap):
                 raise ValueError(f"sensor {k}: pupil must be [{m}][{m}] and valid [{w.n_subap}][{w.n_subap}]")

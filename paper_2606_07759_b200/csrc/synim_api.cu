@@ -321,6 +321,39 @@ int64_t synim_row_offset(const synim_geometry *g, int32_t w)
     return (g && w >= 0 && w < (int)g->wfs.size()) ? g->wfs[w].row_x : -1;
 }
 
+// Dense modes, sensors whose subapertures fit a strip: tiles of the WFS grid (synim_tile_kernel).  A tile is
+// tile_ns strips x tile_nr subaperture rows, about 119 pixels square, shrunk until the bounding box of its
+// pre-image (+ halo, bilinear reach, one pixel of margin, alignment slack) fits a TMA box (<= 256 per side) and the
+// shared-memory budget of two CTAs per SM; then the tile counts are evened out (68 rows -> 4 x 17, not 16+...+4).
+// Returns false if not even a 1 x 1 tile fits (extreme magnification): the caller falls back to source-space pieces.
+struct TilePlan { int ns, nr, pitch, h; };
+static bool plan_tiles(const synim::WfsDev &d, size_t budget_floats, TilePlan *out)
+{
+    const int strip_px = d.spb * d.n_pix, n_strips = (d.n_subap + d.spb - 1) / d.spb;
+    auto box = [&](int ns, int nr, int *pitch, int *h) {
+        const double wt = (double)std::min(ns * strip_px, d.M) + 1.0, ht = (double)std::min(nr * d.n_pix, d.M) + 2.0;   // phi pixels - 1 (one more row: look-ahead)
+        const double ex = std::fabs(d.fwd[0]) * wt + std::fabs(d.fwd[1]) * ht, ey = std::fabs(d.fwd[3]) * wt + std::fabs(d.fwd[4]) * ht;
+        if (!(ex < 1.0e6) || !(ey < 1.0e6)) { *pitch = *h = 1 << 20; return; }
+        *pitch = ((int)std::ceil(ex) + 8 + 3) & ~3;   // floor(cmin)-1-slack(<=3) .. floor(cmax)+2
+        *h = (int)std::ceil(ey) + 5;
+    };
+    int ns = std::max(1, std::min(n_strips, (119 + strip_px / 2) / strip_px));
+    int nr = std::max(1, std::min(d.n_subap, (119 + d.n_pix / 2) / d.n_pix));
+    int pitch = 0, h = 0;
+    while (true) {
+        box(ns, nr, &pitch, &h);
+        if (pitch <= 256 && h <= 256 && (size_t)pitch * h + 3 * (size_t)ns * d.spb * nr <= budget_floats) break;
+        if (ns == 1 && nr == 1) return false;
+        if (nr > 1 && (nr * d.n_pix >= ns * strip_px || ns == 1)) --nr; else --ns;
+    }
+    const int ty = (d.n_subap + nr - 1) / nr, tx = (n_strips + ns - 1) / ns;
+    nr = (d.n_subap + ty - 1) / ty;
+    ns = (n_strips + tx - 1) / tx;
+    box(ns, nr, &pitch, &h);
+    out->ns = ns; out->nr = nr; out->pitch = pitch; out->h = h;
+    return true;
+}
+
 // The launch behind both entry points.  The cube may be PACKED (synim_interaction_matrix_host): mode m
 // then holds only the neighbourhood of its support, cube_ny x cube_nx pixels whose pixel (0, 0) is source
 // pixel d_origin[m] = (ox, oy); bboxes and affine maps stay in source-grid coordinates.
@@ -424,15 +457,14 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         return fail(SYNIM_ERR_CUDA, "synim_interaction_matrix: %zu bytes of shared memory exceed the device limit", smem);
 
     // ---- launches ------------------------------------------------------------------------------
-    // Dense modes: the pieces of a mode are spread over `chunks` CTAs that add into one column, so the
-    // column is cleared first (one strided memset).  Compact modes: the CTA that owns the column writes
-    // its zeros itself.
+    // Compact modes: the CTA that owns a column writes its zeros itself.  Dense modes: sensors whose subapertures
+    // fit a strip go through the tile kernel (output-stationary: every slope stored once); the others (giant
+    // subapertures, or a map so magnified that no tile fits) through source-space pieces spread over `chunks` CTAs
+    // that add into the column, whose rows are cleared first (one strided memset per group).
     int chunks = 1;
     if (dense) {
         const int npieces = ((nx - 1 + cap_w) / cap_w) * ((ny - 1 + cap_h) / cap_h);
         chunks = std::max(1, std::min(npieces, 32));   // (2 .. 64 measured at config 5: 12.3 .. 9.6 ms, flat from 16 on)
-        if (ld == g->rows) SYNIM_CUDA(cudaMemsetAsync(d_out, 0, sizeof(float) * (size_t)g->rows * n_modes, s));
-        else SYNIM_CUDA(cudaMemset2DAsync(d_out, sizeof(float) * (size_t)ld, 0, sizeof(float) * (size_t)g->rows, n_modes, s));
     }
     for (const auto &gr : groups) {
         const int w0 = gr.first, nw = gr.second - gr.first;
@@ -441,13 +473,71 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.origin = d_origin; p.out = d_out; p.ld = ld;
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
         p.addr_bias = 0x4B400000u << 2;
+        for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
+        if (dense && dev[w0].spb > 0) {
+            // two CTAs per SM: half the SM's shared memory less the per-CTA reserve and the static part
+            const size_t budget = (synim::max_dynamic_smem() + 1024) / 2 - 2048 - 8192;   // (8 KB: the warps' scratch)
+            bool fits = true;
+            int tiles = 0, box_floats = 0, tab = 0;
+            for (int w = 0; w < nw && fits; ++w) {
+                TilePlan tp;
+                fits = plan_tiles(p.wfs[w], budget / sizeof(float), &tp);
+                if (!fits) break;
+                synim::WfsDev &d = p.wfs[w];
+                d.tile_ns = tp.ns; d.tile_nr = tp.nr; d.box_pitch = tp.pitch; d.box_h = tp.h;
+                d.tiles_x = ((d.n_subap + d.spb - 1) / d.spb + tp.ns - 1) / tp.ns;
+                d.tiles_y = (d.n_subap + tp.nr - 1) / tp.nr;
+                d.tile_first = tiles;
+                tiles += d.tiles_x * d.tiles_y;
+                d.tab_off = 0; d.tab_cap = 2 * tp.ns * d.spb * tp.nr;
+                box_floats = std::max(box_floats, tp.pitch * tp.h);
+                tab = std::max(tab, d.tab_cap);
+            }
+            if (fits) {
+                synim::TileMaps maps;
+                std::memset(&maps, 0, sizeof(maps));
+                static_assert(sizeof(CUtensorMap) == 128, "TileMaps holds 128-byte descriptors");
+                for (int w = 0; w < nw; ++w) {
+                    CUtensorMap tm;
+                    st = encode_cube_map(d_influence, n_modes, cube_ny, cube_nx, p.wfs[w].box_pitch, p.wfs[w].box_h, &tm);
+                    if (st != SYNIM_OK) return st;
+                    std::memcpy(maps.m[w], &tm, sizeof(tm));
+                }
+                // the kernel's layout: [ box | table | rows ], the box region sized for the largest sensor
+                p.patch_pitch = box_floats; p.patch_h = 1; p.patch_pitchf = (float)box_floats;
+                p.tab_floats = (tab + 3) & ~3;
+                p.tiles_total = tiles;
+                const size_t tsmem = sizeof(float) * ((size_t)box_floats + (size_t)p.tab_floats) + sizeof(int) * (size_t)(p.tab_floats / 2);
+                for (int m0 = 0; m0 < n_modes; m0 += 65535) {   // grid.y holds the modes
+                    synim::ImParams q = p;
+                    q.n_modes = std::min(65535, n_modes - m0);
+                    q.out = d_out + (size_t)m0 * (size_t)ld;
+                    if (m0 > 0) {   // the descriptors address modes from the cube's start: re-encode on the batch
+                        const float *sub = d_influence + (size_t)m0 * (size_t)cube_ny * (size_t)cube_nx;
+                        for (int w = 0; w < nw; ++w) {
+                            CUtensorMap tm;
+                            st = encode_cube_map(sub, q.n_modes, cube_ny, cube_nx, p.wfs[w].box_pitch, p.wfs[w].box_h, &tm);
+                            if (st != SYNIM_OK) return st;
+                            std::memcpy(maps.m[w], &tm, sizeof(tm));
+                        }
+                    }
+                    SYNIM_CUDA(synim::launch_tiles(q, maps, tsmem, mode == SYNIM_SLOPES_GTILT, s));
+                }
+                continue;
+            }
+            for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];   // no tile fits: source-space pieces
+        }
         p.patch_pitchf = (float)patch_pitch;
         p.patch_pitch = patch_pitch; p.patch_h = patch_h;
-        for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
         p.tab_floats = nw > 0 ? (dev[w0 + nw - 1].tab_off + dev[w0 + nw - 1].tab_cap + 3) & ~3 : 0;
         p.chunks = chunks;
         if (dense) {
             p.zero_begin = 0; p.zero_count = 0;
+            const int r_begin = g->wfs[w0].row_x;
+            const WfsHost &last = g->wfs[w0 + nw - 1];
+            const size_t r_count = (size_t)(last.row_x + 2 * last.n_valid - r_begin);
+            if (r_count > 0)
+                SYNIM_CUDA(cudaMemset2DAsync(d_out + r_begin, sizeof(float) * (size_t)ld, 0, sizeof(float) * r_count, n_modes, s));
         } else {
             p.zero_begin = g->wfs[w0].row_x;
             const WfsHost &last = g->wfs[w0 + nw - 1];

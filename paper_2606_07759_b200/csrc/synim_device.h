@@ -34,6 +34,11 @@ struct WfsDev {
     unsigned npx_magic;      // ceil(2^32 / n_pix): x / n_pix = umulhi(x, npx_magic) for the pixel indices met here
     int row_x, row_y;        // first row of the x / y slopes of this sensor inside a column
     int tab_off, tab_cap;    // this sensor's slice of the CTA's slope table (floats)
+    // dense modes, tiles of the WFS grid (synim_tile_kernel): a tile is tile_ns strips x tile_nr subaperture rows
+    int tile_ns, tile_nr;    // strips (of spb subapertures) and subaperture rows per tile
+    int tiles_x, tiles_y;    // tiles across / down the sensor
+    int tile_first;          // index of this sensor's first tile among the launch's tiles of one mode
+    int box_pitch, box_h;    // the staged pre-image of a tile: floats per row (multiple of 4), rows
 };
 
 struct ImParams {
@@ -51,13 +56,23 @@ struct ImParams {
     float patch_pitchf;         // patch_pitch as float (an FFMA operand straight from constant memory)
     unsigned addr_bias;         // (bits of 1.5*2^23) << 2 mod 2^32, see process_strip
     int tab_floats;             // size of the CTA's slope table (multiple of 4)
+    int tiles_total;            // tile kernel: tiles of one mode over all sensors of the launch
     WfsDev wfs[kMaxWfsPerLaunch];
+};
+
+// tile kernel: one TMA descriptor per sensor (the boxes differ with the sensors' rotations); 128 bytes each,
+// 64-byte aligned as the hardware wants
+struct alignas(64) TileMaps {
+    unsigned char m[kMaxWfsPerLaunch][128];
 };
 
 // launchers; all asynchronous on `stream`, return the launch status.
 // The hot path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
 // {patch_pitch, patch_h, 1}
 cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream);
+// Dense modes over sensors whose subapertures fit a strip: one CTA per (mode, sensor, tile of the WFS grid);
+// maps.m[w] is sensor w's CUtensorMap over the cube with box {box_pitch, box_h, 1}
+cudaError_t launch_tiles(const ImParams &p, const TileMaps &maps, size_t smem_bytes, bool gtilt, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
                                  float *d_wmap, int *d_subap_row, int *d_error_flag, cudaStream_t stream);
 cudaError_t launch_gtilt_maps(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix, float *d_gx, float *d_gy,

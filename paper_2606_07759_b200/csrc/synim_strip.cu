@@ -47,6 +47,12 @@ namespace {
 #ifndef SYNIM_STRIP_UNROLL
 #define SYNIM_STRIP_UNROLL 1   // unrolling of the row loop
 #endif
+#ifndef SYNIM_TILE_BATCHED_EDGES
+#define SYNIM_TILE_BATCHED_EDGES 1   // 0: the tile kernel combines the lanes of every edge-sum unit with shuffles (comparisons)
+#endif
+#ifndef SYNIM_EDGE_SUM
+#define SYNIM_EDGE_SUM 1       // 0: uniformly lit subapertures take the general path too (for comparisons)
+#endif
 constexpr int kComputeWarps = SYNIM_STRIP_WARPS, kComputeThreads = 32 * kComputeWarps;
 constexpr int kStripThreads = kComputeThreads;
 constexpr int kStripUnroll = SYNIM_STRIP_UNROLL;
@@ -55,6 +61,7 @@ static_assert(2 * kStripRows <= kWmapPadRows, "weight look-ahead runs past the r
 constexpr int kStripCols = kStripMaxCols;     // D columns per strip: lanes 1..30, halo on lanes 0 and 31
 constexpr float kMagicFloor = 12582912.0f;   // 1.5 * 2^23: fadd.rm(x, magic) = magic + floor(x), |x| < 2^22
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kEdgeBatch = 8;                // tile kernel: units whose lane sums are combined in one go (per-warp scratch)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -121,6 +128,7 @@ __device__ __forceinline__ void red_shared_f32(uint32_t addr, float v)
     asm volatile("red.shared.add.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
 }
 __device__ __forceinline__ void sts_f32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
+__device__ __forceinline__ void sts_s32(uint32_t addr, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
 __device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 template <int NT>
 __device__ __forceinline__ void zero_fill(float *dst, int n, int tid)
@@ -213,21 +221,48 @@ __device__ __forceinline__ int div_npx(int x, int npx, unsigned magic) { return 
 // kGtilt: the G-tilt estimator (reading R13) instead of the numerical derivative: the slopes are then two
 // weighted sums of phi itself (coefficient maps gx, gy: +-1/den on the first / last valid pixel of every
 // pixel row / column of a subaperture), so the stencil and its shuffles drop out (general path only).
-template <bool kGtilt, bool kAligned>
+//
+// kTile (dense modes, synim_tile_kernel): the strip is a piece of a tile of the WFS grid whose whole pre-image
+// (halo and bilinear reach included) is staged, so (a) no sample can leave the staged box: no range test, no row
+// pruning; (b) coordinates are taken relative to the pre-image of the strip's own centre (an integer source pixel
+// folded into the address base), which keeps |col|, |row| below ~64 and their float32 spacing below 4e-6 pixels
+// however large the box is; (c) a unit none of whose subapertures is valid is SKIPPED (nothing is sampled for it).
+template <bool kGtilt, bool kAligned, bool kTile>
 __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
-                                              uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp)
+                                              uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp,
+                                              uint32_t scr = 0u)
 {
-    constexpr bool kEdge = kAligned && !kGtilt;   // the edge-sum path exists
+    static_assert(!kTile || kAligned, "tiles are made of aligned strips");
+    constexpr bool kEdge = kAligned && !kGtilt && SYNIM_EDGE_SUM != 0;   // the edge-sum path exists
     constexpr int kRows = kStripRows;
     static_assert(kRows == 2, "the segment loops are written for two rows per iteration");
     const int lane = threadIdx.x & 31;
     const int nR = i1 - i0 + 1;   // D rows; phi row rr (0 .. nR+1) is absolute row i0-1+rr
     const int jcol = jA - 1 + lane;
 
-    // S1: float64 per-lane base, then float32 tile-local offsets
-    const double jl = (double)jcol, ib = (double)(i0 - 1);
-    const float bc = (float)(W.fwd[0] * jl + W.fwd[1] * ib + W.fwd[2] - (double)cb.x0);
-    const float br = (float)(W.fwd[3] * jl + W.fwd[4] * ib + W.fwd[5] - (double)cb.y0);
+    // S1: float64 per-lane base, then float32 tile-local offsets.  (kTile samples without a range test: the lanes
+    // beyond the strip's right halo column stay on it, inside the staged pre-image.)
+    const double jl = (double)(kTile ? min(jcol, jA + nC) : jcol);
+    float bc = (float)(W.fwd[0] * jl + W.fwd[1] * (double)(i0 - 1) + W.fwd[2] - (double)cb.x0);
+    float br = (float)(W.fwd[3] * jl + W.fwd[4] * (double)(i0 - 1) + W.fwd[5] - (double)cb.y0);
+    // byte address of element 0 minus (bits of the magic number << 2) mod 2^32.  The bias is a kernel
+    // parameter, not a literal, so that ptxas keeps the difference in one register and an address is one LEA
+    uint32_t cbase = cb.base - addr_bias;
+    int roff = 0;   // phi row rr (counted from absolute row i0-1) is sampled at rf = rr - roff
+    // kTile: coordinates are re-based every few units on the pre-image of the centre of the rows ahead (an integer
+    // source pixel, folded into the address base) and counted from their first row: |col|, |row| and rf stay below
+    // ~40, so the float32 roundings of the base, of the product a1*rf and of the sum stay near 2e-6 pixels however
+    // tall the strip is.  rr0 .. rr1: the phi rows (counted from i0-1) sampled until the next call.
+    auto rebase = [&](int rr0, int rr1) {
+        const double jm = (double)jA + 0.5 * (double)nC, im = (double)(i0 - 1) + 0.5 * (double)(rr0 + rr1);
+        const int xc = __double2int_rn(W.fwd[0] * jm + W.fwd[1] * im + W.fwd[2] - (double)cb.x0);
+        const int yc = __double2int_rn(W.fwd[3] * jm + W.fwd[4] * im + W.fwd[5] - (double)cb.y0);
+        const double ib = (double)(i0 - 1 + rr0);
+        bc = (float)(W.fwd[0] * jl + W.fwd[1] * ib + W.fwd[2] - (double)(cb.x0 + xc));
+        br = (float)(W.fwd[3] * jl + W.fwd[4] * ib + W.fwd[5] - (double)(cb.y0 + yc));
+        cbase = cb.base + (uint32_t)(yc * cb.pitch + xc) * 4u - addr_bias;
+        roff = rr0;
+    };
     const float a1 = (float)W.fwd[1], a4 = (float)W.fwd[4];
     const float cwf = (float)cb.cw, chf = (float)cb.ch;
 
@@ -237,7 +272,8 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     const float bcL = __shfl_sync(kFull, bc, 0), brL = __shfl_sync(kFull, br, 0);
     const float bcR = __shfl_sync(kFull, bc, nC + 1), brR = __shfl_sync(kFull, br, nC + 1);
     int first = 0x7fffffff, last = -1;
-    for (int g = 0; g < nR + 2; g += 32) {
+    if (kTile) { first = 0; last = nR + 1; }
+    for (int g = 0; !kTile && g < nR + 2; g += 32) {
         const int rr = g + lane;
         const float rf = (float)rr;
         const float cl = fmaf(a1, rf, bcL), cr = fmaf(a1, rf, bcR);
@@ -260,6 +296,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     const int npx = W.n_pix, n_subap = W.n_subap;
     const bool isD = lane >= 1 && lane <= nC;
     const int seg = isD ? div_npx(jcol, npx, W.npx_magic) : -1;
+    const int seg_first = div_npx(jA, npx, W.npx_magic);   // (aligned strips start on a subaperture boundary)
     const int segL = __shfl_up_sync(kFull, seg, 1);
     const bool head = isD && (lane == 1 || segL != seg);
     unsigned okm = 0;
@@ -280,17 +317,24 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
 
     // bit u of genmask: unit a_first+u needs the general path (lane u looks at the strip's subapertures of
     // its unit; units beyond 32 are simply taken as general)
-    unsigned genmask = 0xffffffffu;
-    if (kEdge) {
+    // bit u of skipmask (kTile): none of the strip's subapertures of unit a_first+u is valid
+    unsigned genmask = 0xffffffffu, skipmask = 0u;
+    if (kEdge || kTile) {
         const int bA = div_npx(jA, npx, W.npx_magic), nsb = div_npx(nC, npx, W.npx_magic);
         const int a_mine = a_first + lane;
-        bool gflag = false;
+        bool gflag = false, vflag = false;
         if (a_mine < n_subap) {
             const int *rp = W.subap_row + a_mine * n_subap + bA;
             for (int q = 0; q < nsb; ++q)
-                if (bA + q < n_subap) { const int c = __ldg(rp + q); gflag = gflag || (c >= 0 && (c & kSubapGeneral) != 0); }
+                if (bA + q < n_subap) {
+                    const int c = __ldg(rp + q);
+                    gflag = gflag || (c >= 0 && (c & kSubapGeneral) != 0);
+                    vflag = vflag || c >= 0;
+                }
         }
-        genmask = __ballot_sync(kFull, gflag);
+        if (kEdge) genmask = __ballot_sync(kFull, gflag);
+        if (kTile) skipmask = __ballot_sync(kFull, a_mine < n_subap && !vflag);
+        genmask &= ~skipmask;
     }
 
     // S3 (columns), general path: segmented sum over the lanes of a subaperture, then one shared-memory
@@ -346,17 +390,23 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // overlap: the kernel is latency-bound otherwise (ncu, round 1).
     const uint32_t cw_bits = __float_as_uint(cwf), ch_bits = __float_as_uint(chf);
     const float pitchf = cb.pitchf;
-    // byte address of element 0 minus (bits of the magic number << 2) mod 2^32.  The bias is a kernel
-    // parameter, not a literal, so that ptxas keeps the difference in one register and an address is one LEA
-    const uint32_t cbase = cb.base - addr_bias;
     const uint32_t rpitch4 = (uint32_t)cb.pitch * 4u;
     auto sample = [&](float rf) -> float {
         const float col = fmaf(a1, rf, bc), row = fmaf(a4, rf, br);
         const float tc = __fadd_rd(col, kMagicFloor), tr = __fadd_rd(row, kMagicFloor);   // magic + floor
         const float fx = col - (tc - kMagicFloor), fy = row - (tr - kMagicFloor);
-        // magic + c0 + r0*pitch is exact: its mantissa is the element index
+        // magic + c0 + r0*pitch is exact: its mantissa is the element index (a negative index borrows from
+        // the mantissa's leading bit: still exact, and the address arithmetic is modulo 2^32)
         const uint32_t idx = __float_as_uint(fmaf(tr - kMagicFloor, pitchf, tc));
         const uint32_t at = idx * 4u + cbase;
+        if (kTile) {   // the whole pre-image of the tile is staged: nothing to test
+#ifdef SYNIM_CHECKS
+            if (at < cb.base || at + rpitch4 + 8u > cb.limit) __trap();
+#endif
+            const float v00 = lds_f32(at), v01 = lds_f32(at + 4u), v10 = lds_f32(at + rpitch4), v11 = lds_f32(at + rpitch4 + 4u);
+            const float t = fmaf(fx, v01 - v00, v00), u = fmaf(fx, v11 - v10, v10);
+            return fmaf(fy, u - t, t);
+        }
 #ifdef SYNIM_CHECKS   // debug build: a sample that passes the range test must lie inside the staged box
         if (__float_as_uint(col) < cw_bits && __float_as_uint(row) < ch_bits &&
             (at < cb.base || at + rpitch4 + 8u > cb.limit)) __trap();
@@ -394,14 +444,25 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     while (d <= d_hi) {
         // the segment: units of one kind from the current one on; D rows d .. d_end
         const int u = a_cur - a_first;
-        const bool gen = !kEdge || u >= 32 || ((genmask >> u) & 1u);
+        const bool skip = kTile && u < 32 && ((skipmask >> u) & 1u);
+        const bool gen = !skip && (!kEdge || u >= 32 || ((genmask >> u) & 1u));
         int d_end = d_hi;
-        if (kEdge && u < 32) {
-            const unsigned other = (gen ? ~genmask : genmask) >> u;   // bit k: unit u+k is of the other kind
+        if ((kEdge || kTile) && u < 32) {
+            const unsigned mine = skip ? skipmask : (gen ? genmask : ~(genmask | skipmask));
+            const unsigned other = ~mine >> u;   // bit k: unit u+k is of another kind
             if (other) d_end = min(d_hi, (a_cur + __ffs(other) - 1) * npx - i0);   // last D row before that unit
         }
-        float rf = (float)(d + 1);
-        float pmA = sample((float)(d - 1)), pmB = sample((float)d);   // phi[d-1], phi[d]
+        if (skip) {   // whole units (a tile's strips start and end on unit boundaries): nothing to sample
+            const int nu = (d_end - d + 1) / npx;
+            a_cur += nu; tent += tstep * (uint32_t)nu;
+            d = d_end + 1;
+            continue;
+        }
+        constexpr int kRebaseUnits = 4;   // kTile: units between two re-basings of the coordinates
+        const int rebase_rows = kRebaseUnits * npx;
+        if (kTile) rebase(d - 1, min(d_end, d - 1 + rebase_rows) + 1);
+        float rf = (float)(d + 1 - roff);
+        float pmA = sample((float)(d - 1 - roff)), pmB = sample((float)(d - roff));   // phi[d-1], phi[d]
         if (gen) {
             const float *wm = kGtilt ? W.gx : W.wmap, *wm2 = kGtilt ? W.gy : W.wmap;
             // weight map offsets (elements).  The map has kWmapPadRows rows of zeros below row M-1: halo lanes
@@ -420,13 +481,17 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
             for (; d <= d_end; d += kRows) {
 #pragma unroll
                 for (int q = 0; q < (kComputeWarps >= 4 ? 1 : 4 / kComputeWarps); ++q) zp.step();
+                if (kTile && d + 1 - roff > rebase_rows) {   // (phi[d-1], phi[d] are in registers already)
+                    rebase(d + 1, min(d_end, d + rebase_rows) + 2);
+                    rf = 0.0f;
+                }
                 float cur[kRows];   // phi[d+1 .. d+kRows]
 #pragma unroll
                 for (int k = 0; k < kRows; ++k) cur[k] = sample(rf + (float)k);
                 rf += (float)kRows;
                 // D rows d, d+1: D_y from registers, D_x from the neighbouring lanes.  A row past d_hi has D = 0
                 // exactly (or a weight from the rows of zeros); a row past d_end is the next segment's.
-                const bool two = !kEdge || d + 1 <= d_end;
+                const bool two = !(kEdge || kTile) || d + 1 <= d_end;
 #pragma unroll
                 for (int k = 0; k < kRows; ++k) {
                     const float mid = k == 0 ? pmB : cur[k - 1];                         // phi[d+k]
@@ -455,6 +520,69 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
                 }
             }
             if (rem > 0 && d_end == d_hi) { flush_general(sx, sy); rem = 0; }   // the walk ended inside a unit
+        } else if (kTile && SYNIM_TILE_BATCHED_EDGES != 0) {
+            // Edge-sum units of a tile: whole units, four rows in flight.  Per unit and lane only the column sum cs
+            // and the difference v of the two row pairs are formed; they are parked in the warp's scratch
+            // ([kEdgeBatch units][33] floats each) and the lanes are combined kEdgeBatch units at a time
+            // (edge_phase2): a handful of instructions per unit instead of five shuffle steps.
+            const int nu = (d_end - d + 1) / npx;
+            const int nsb = div_npx(nC, npx, W.npx_magic);
+            auto edge_phase2 = [&](int a_start, int cnt) {
+                __syncwarp();
+                for (int t = lane; t < cnt * nsb; t += 32) {
+                    const int uu = t / nsb, sb = t - uu * nsb;
+                    const uint32_t rc = scr + (uint32_t)(uu * 33 + 1 + sb * npx) * 4u;       // cs of the subaperture's first column
+                    const uint32_t rv = rc + (uint32_t)(kEdgeBatch * 33) * 4u;               // v of it
+                    const uint32_t n4 = (uint32_t)npx * 4u;
+                    const float sx = (lds_f32(rc + n4) + lds_f32(rc + n4 - 4u)) - (lds_f32(rc) + lds_f32(rc - 4u));
+                    float sy = lds_f32(rv);
+                    for (int k = 1; k < npx; ++k) sy += lds_f32(rv + (uint32_t)k * 4u);
+                    const uint32_t te = tab + (uint32_t)((a_start + uu - a0) * nb + (seg_first - b0) + sb) * 8u;
+#ifdef SYNIM_CHECKS
+                    if (te < tab || te + 8u > tab + (uint32_t)W.tab_cap * 4u) __trap();
+#endif
+                    sts_f32(te, sx * wu);
+                    sts_f32(te + 4u, sy * wu);
+                }
+                __syncwarp();
+            };
+            float pairt = pmA + pmB, carry = pmB;   // phi[i0-1] + phi[i0] and phi[i0] of the current unit
+            int slot = 0, a_batch = a_cur;
+            int rr = d + 1;   // next phi row to sample (counted from i0-1)
+            for (int uu = 0; uu < nu; ++uu, rr += npx) {
+                if (uu != 0 && (uu & (kRebaseUnits - 1)) == 0) {
+                    rebase(rr, min(d_end + 1, rr + rebase_rows));
+                    rf = 0.0f;
+                }
+                // rows i0+1 .. i0+n of the unit (the last one is the next unit's first row)
+                float tot = 0.0f, prev = carry, last = carry;
+                int k = 0;
+                for (; k + 4 <= npx; k += 4) {
+                    const float c0 = sample(rf), c1 = sample(rf + 1.0f), c2 = sample(rf + 2.0f), c3 = sample(rf + 3.0f);
+                    rf += 4.0f;
+                    tot += (c0 + c1) + (c2 + c3);
+                    prev = c2; last = c3;
+                }
+                const int r = npx - k;
+                if (r == 3) {
+                    const float c0 = sample(rf), c1 = sample(rf + 1.0f), c2 = sample(rf + 2.0f);
+                    tot += (c0 + c1) + c2; prev = c1; last = c2;
+                } else if (r == 2) {
+                    const float c0 = sample(rf), c1 = sample(rf + 1.0f);
+                    tot += c0 + c1; prev = c0; last = c1;
+                } else if (r == 1) {
+                    const float c0 = sample(rf);
+                    tot += c0; prev = last; last = c0;
+                }
+                rf += (float)r;
+                const float pairb = prev + last;                      // phi[i0+n-1] + phi[i0+n]
+                sts_f32(scr + (uint32_t)(slot * 33 + lane) * 4u, carry + (tot - last));                     // cs
+                sts_f32(scr + (uint32_t)((kEdgeBatch + slot) * 33 + lane) * 4u, pairb - pairt);            // v
+                pairt = pairb; carry = last;
+                if (++slot == kEdgeBatch) { edge_phase2(a_batch, slot); a_batch += slot; slot = 0; }
+            }
+            if (slot) edge_phase2(a_batch, slot);
+            a_cur += nu; tent += tstep * (uint32_t)nu;
         } else {
             float cs = 0.0f;   // sum of phi over the rows of the unit so far
             // phi[i0-1] + phi[i0] of the current unit: both rows lie above the walk (where phi is 0) unless the
@@ -585,10 +713,10 @@ __device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, i
         const uint32_t tab = tab_base + (uint32_t)W.tab_off * 4u;
         if (kAligned) {
             const int bA = b0 + (t - base) * spb;
-            process_strip<kGtilt, true>(W, i0, i1, bA * W.n_pix, min(spb, b0 + nb - bA) * W.n_pix, cb, p.addr_bias, tab, a0, b0, nb, zp);
+            process_strip<kGtilt, true, false>(W, i0, i1, bA * W.n_pix, min(spb, b0 + nb - bA) * W.n_pix, cb, p.addr_bias, tab, a0, b0, nb, zp);
         } else {
             const int jA = j0 + (t - base) * kStripCols;
-            process_strip<kGtilt, false>(W, i0, i1, jA, min(kStripCols, j1 - jA + 1), cb, p.addr_bias, tab, a0, b0, nb, zp);
+            process_strip<kGtilt, false, false>(W, i0, i1, jA, min(kStripCols, j1 - jA + 1), cb, p.addr_bias, tab, a0, b0, nb, zp);
         }
     }
 }
@@ -742,6 +870,125 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
     if (!multi && npieces > 0) scatter_table<false, kStripThreads>(p, s_win, tab_base, krow_base, colp, tid);
 }
 
+
+// ---- dense modes: tiles of the WFS grid -------------------------------------------------------------------------
+// A dense mode has no support to skip, so the work is cut in WFS space, output-stationary: one CTA per (mode, sensor,
+// tile of tile_ns strips x tile_nr subaperture rows).  The tile's pre-image under the sensor's map -- the bounding
+// box of its four corners, plus the halo, the reach of a bilinear sample and the alignment slack -- is staged by ONE
+// TMA box load (the sensor's own descriptor: the box of a sensor rotated by 60 degrees is twice that of an unrotated
+// one), the warps take (strip, rows) pieces of the tile, and every slope of the tile is stored exactly once, by this
+// CTA, with plain streaming stores: no memset, no atomics.  CTAs are ordered mode-major, so a mode's image is read
+// from HBM once and served from L2 to the other tiles and sensors (the cube is fetched once for all
+// WFS).  Units of invalid subapertures (outside the pupil) are skipped.
+#ifndef SYNIM_TILE_WARPS
+#define SYNIM_TILE_WARPS 4
+#endif
+constexpr int kTileWarps = SYNIM_TILE_WARPS, kTileThreads = 32 * kTileWarps;
+constexpr int kTileScratchFloats = 2 * kEdgeBatch * 33;   // per warp: cs and v of kEdgeBatch units, one float per lane (+1 pad)
+
+__device__ __forceinline__ void tma_load_box_plain(void *dst, const void *map, uint64_t *bar, int x, int y, int z)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z)
+        : "memory");
+}
+
+// grid: x = tile of the mode (all sensors of the launch), y = mode -- the tiles of a mode are neighbours in launch order
+template <bool kGtilt>
+__global__ void __launch_bounds__(kTileThreads, 2) synim_tile_kernel(const __grid_constant__ ImParams p,
+                                                                     const __grid_constant__ TileMaps maps)
+{
+    // [ TMA box: box_pitch x box_h floats of this sensor (<= patch_pitch floats) | table | rows | scratch ]
+    extern __shared__ __align__(128) float patch[];
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ int s_next;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int mode = blockIdx.y;
+    int t = blockIdx.x;
+    int w = 0;
+    while (w + 1 < p.n_wfs && t >= p.wfs[w + 1].tile_first) ++w;
+    const WfsDev &W = p.wfs[w];
+    t -= W.tile_first;
+    const int ty = t / W.tiles_x, tx = t - ty * W.tiles_x;
+    const int spb = W.spb, npx = W.n_pix, n_subap = W.n_subap;
+    const int b0 = tx * W.tile_ns * spb, nb = min(W.tile_ns * spb, n_subap - b0);
+    const int a0 = ty * W.tile_nr, na = min(W.tile_nr, n_subap - a0);
+    const uint32_t raw_base = smem_u32(patch);
+    const uint32_t tab_base = raw_base + (uint32_t)p.patch_pitch * 4u;
+    const uint32_t krow_base = tab_base + (uint32_t)p.tab_floats * 4u;
+    const uint32_t scr = krow_base + (uint32_t)(p.tab_floats >> 1) * 4u + (uint32_t)(warp * kTileScratchFloats) * 4u;
+
+    // the IM rows of the tile's subapertures; a tile without a valid one has nothing to compute or to store
+    int any = 0;
+    for (int ra = warp; ra < na; ra += kTileWarps)
+        for (int rb = lane; rb < nb; rb += 32) {
+            const int k = __ldg(W.subap_row + (a0 + ra) * n_subap + b0 + rb);
+            sts_s32(krow_base + (uint32_t)(ra * nb + rb) * 4u, k);
+            any |= (k >= 0);
+        }
+    if (!__syncthreads_or(any)) return;
+
+    // pre-image of the tile's phi pixels (halo included): bounding box of the four corners, float64
+    const double jl = (double)(b0 * npx - 1), jh = (double)((b0 + nb) * npx);
+    const double il = (double)(a0 * npx - 1), ih = (double)((a0 + na) * npx + 1);   // (+1: the general path's row look-ahead)
+    const double cmin = W.fwd[2] + fmin(W.fwd[0] * jl, W.fwd[0] * jh) + fmin(W.fwd[1] * il, W.fwd[1] * ih);
+    const double rmin = W.fwd[5] + fmin(W.fwd[3] * jl, W.fwd[3] * jh) + fmin(W.fwd[4] * il, W.fwd[4] * ih);
+    const double lim = 1.0e9;
+    const int x0 = ((int)floor(fmax(fmin(cmin, lim), -lim)) - 1) & ~3;   // one pixel of margin, 16-byte aligned
+    const int y0 = (int)floor(fmax(fmin(rmin, lim), -lim)) - 1;
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        fence_barrier_init();
+        fence_proxy_async();
+        mbar_expect_tx(&bar, (uint32_t)(W.box_pitch * W.box_h) * 4u);
+        tma_load_box_plain(patch, &maps.m[w][0], &bar, x0, y0, mode);
+        s_next = 0;
+    }
+    for (int e = tid; e < na * nb * 2; e += kTileThreads) sts_f32(tab_base + (uint32_t)e * 4u, 0.0f);
+    __syncthreads();   // mbarrier initialised, table cleared
+
+    CellBox cb;
+    cb.x0 = x0; cb.y0 = y0; cb.cw = W.box_pitch; cb.ch = W.box_h;
+    cb.base = raw_base; cb.pitch = W.box_pitch; cb.pitchf = (float)W.box_pitch;
+    cb.limit = raw_base + (uint32_t)(W.box_pitch * W.box_h) * 4u;
+    cb.s_lo = cb.d_lo = -3.0e38f; cb.s_hi = cb.d_hi = 3.0e38f;
+    ZeroPacer zp;
+    zp.base = nullptr; zp.next = 0; zp.end = 0;
+
+    // pieces: strip s of the tile x chunk c of its subaperture rows (one chunk unless the tile has fewer strips than
+    // the CTA has warps), first come, first served
+    const int ns = (nb + spb - 1) / spb;
+    int nch = max(1, min(na, kTileWarps / ns));
+    const int cr = (na + nch - 1) / nch;
+    nch = (na + cr - 1) / cr;
+    const int total = ns * nch;
+    mbar_wait(&bar, 0);
+    while (true) {
+        int it = 0;
+        if (lane == 0) it = atomicAdd(&s_next, 1);
+        it = __shfl_sync(kFull, it, 0);
+        if (it >= total) break;
+        const int c = it / ns, sidx = it - c * ns;
+        const int bA = b0 + sidx * spb, aA = a0 + c * cr, aE = min(aA + cr, a0 + na);
+        process_strip<kGtilt, true, true>(W, aA * npx, aE * npx - 1, bA * npx, min(spb, b0 + nb - bA) * npx, cb, p.addr_bias,
+                                          tab_base, a0, b0, nb, zp, scr);
+    }
+    __syncthreads();   // table complete
+
+    // S4: every slope of the tile, once (zeros included); consecutive valid subapertures of a subaperture row are
+    // consecutive IM rows
+    float *colp = p.out + (long long)mode * p.ld;
+    const int n_sub = na * nb;
+    for (int e = tid; e < 2 * n_sub; e += kTileThreads) {
+        const int axis = e >= n_sub, q = axis ? e - n_sub : e;
+        const int k = lds_s32(krow_base + (uint32_t)q * 4u);
+        if (k < 0) continue;
+        const float v = lds_f32(tab_base + (uint32_t)(2 * q + axis) * 4u);
+        __stcs(colp + (axis ? W.row_y : W.row_x) + (k & kSubapRowMask), v * W.scale);
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream)
@@ -768,6 +1015,29 @@ cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_
     memcpy(&tm, tensor_map, sizeof(tm));
     note_launch();
     kernel<<<dim3((unsigned)p.n_modes, (unsigned)(p.chunks > 0 ? p.chunks : 1)), kStripThreads, smem_bytes, stream>>>(p, tm);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_tiles(const ImParams &p, const TileMaps &maps, size_t smem_bytes, bool gtilt, cudaStream_t stream)
+{
+    if (p.n_modes <= 0 || p.tiles_total <= 0) return cudaSuccess;
+    for (int w = 0; w < p.n_wfs; ++w)
+        if (p.wfs[w].spb <= 0) return cudaErrorInvalidValue;
+    if (p.n_modes > 65535) return cudaErrorInvalidValue;   // (the host splits larger batches)
+    auto kernel = gtilt ? synim_tile_kernel<true> : synim_tile_kernel<false>;
+    static size_t granted[2][64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    smem_bytes += sizeof(float) * (size_t)(kTileWarps * kTileScratchFloats);
+    size_t &have = granted[gtilt ? 1 : 0][dev & 63];
+    if (smem_bytes > have) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return e;
+        have = smem_bytes;
+    }
+    note_launch();
+    kernel<<<dim3((unsigned)p.tiles_total, (unsigned)p.n_modes), kTileThreads, smem_bytes, stream>>>(p, maps);
     return cudaGetLastError();
 }
 

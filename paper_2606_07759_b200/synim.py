@@ -109,7 +109,7 @@ def launch_count() -> int:
 
 def hot_kernel_name(dense: bool) -> str:
     """Name of the kernel that dominates a step (for reports; the launch lists under profiles/ show it)."""
-    return "synim_strip_kernel<false> (dense modes: source-space pieces)" if dense else "synim_strip_kernel<false>"
+    return "synim_tile_kernel<false> (dense modes: tiles of the WFS grid)" if dense else "synim_strip_kernel<false, true>"
 
 
 def last_error() -> str:

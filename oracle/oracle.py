@@ -48,6 +48,15 @@ def _load():
             ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
             ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, f64p, ctypes.c_double,
             ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p]
+        lib.synim_oracle_wfs_repair.restype = ctypes.c_int
+        lib.synim_oracle_wfs_repair.argtypes = [
+            ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+            ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, f64p,
+            ctypes.c_double, ctypes.c_int32, ctypes.c_void_p]
+        lib.synim_oracle_repair_screen.restype = ctypes.c_int
+        lib.synim_oracle_repair_screen.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
+                                                   ctypes.c_int32, f64p, ctypes.c_double, ctypes.c_void_p,
+                                                   ctypes.c_void_p, ctypes.c_void_p]
         lib.synim_oracle_resample.restype = ctypes.c_int
         lib.synim_oracle_resample.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
                                               f64p, ctypes.c_int32, ctypes.c_void_p]
@@ -84,6 +93,56 @@ def resample(g: np.ndarray, m: int, a: Sequence[float], halo: bool = False) -> n
     return out
 
 
+REPAIR_THRESHOLD = 0.999999   #: the paper's example value
+
+
+def repair_screen(g: np.ndarray, mask: np.ndarray, m: int, a: Sequence[float],
+                  threshold: float = REPAIR_THRESHOLD):
+    """Edge repair of one mode: (phi_repaired float64, core uint8, ring uint8), each on the
+    [M+2][M+2] halo grid of pixels -1..M."""
+    g = np.ascontiguousarray(g, dtype=np.float32)
+    mask = np.ascontiguousarray(mask, dtype=np.float32)
+    assert g.shape == mask.shape
+    phi = np.empty((m + 2, m + 2), dtype=np.float64)
+    core = np.empty((m + 2, m + 2), dtype=np.uint8)
+    ring = np.empty((m + 2, m + 2), dtype=np.uint8)
+    aa = (ctypes.c_double * 6)(*[float(v) for v in a])
+    rc = _load().synim_oracle_repair_screen(g.ctypes.data, mask.ctypes.data, g.shape[0], g.shape[1], m, aa,
+                                            float(threshold), phi.ctypes.data, core.ctypes.data, ring.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle repair failed ({rc})")
+    return phi, core, ring
+
+
+def slopes_wfs_repair(cube: np.ndarray, mask: np.ndarray, pupil: np.ndarray, n_subap: int, n_pix: int,
+                      valid: np.ndarray, a: Sequence[float], scale: float = 1.0,
+                      threshold: float = REPAIR_THRESHOLD, modes: Optional[Sequence[int]] = None,
+                      n_threads: int = 0) -> np.ndarray:
+    """Edge-repaired numerical-derivative slopes of the selected modes for one WFS:
+    float64 [n_sel][2*n_valid] (x then y)."""
+    cube = np.ascontiguousarray(cube, dtype=np.float32)
+    mask = np.ascontiguousarray(mask, dtype=np.float32)
+    pupil = np.ascontiguousarray(pupil, dtype=np.float32)
+    valid = np.ascontiguousarray(valid, dtype=np.uint8)
+    n_tot, ny, nx = cube.shape
+    assert mask.shape == (ny, nx)
+    assert pupil.shape == (n_subap * n_pix, n_subap * n_pix) and valid.shape == (n_subap, n_subap)
+    if modes is None:
+        idx_p, n_sel = None, n_tot
+    else:
+        idx = np.ascontiguousarray(modes, dtype=np.int32)
+        idx_p, n_sel = idx.ctypes.data, idx.size
+    nv = int(valid.sum())
+    out = np.zeros((n_sel, 2 * nv), dtype=np.float64)
+    aa = (ctypes.c_double * 6)(*[float(v) for v in a])
+    rc = _load().synim_oracle_wfs_repair(cube.ctypes.data, n_tot, idx_p, n_sel, ny, nx, mask.ctypes.data,
+                                         float(threshold), pupil.ctypes.data, n_subap, n_pix, valid.ctypes.data, aa,
+                                         float(scale), int(n_threads), out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle failed ({rc})")
+    return out
+
+
 def slopes_wfs(cube: np.ndarray, pupil: np.ndarray, n_subap: int, n_pix: int, valid: np.ndarray,
                a: Sequence[float], scale: float = 1.0, mode: int = ND,
                modes: Optional[Sequence[int]] = None, n_threads: int = 0) -> np.ndarray:
@@ -111,16 +170,25 @@ def slopes_wfs(cube: np.ndarray, pupil: np.ndarray, n_subap: int, n_pix: int, va
 
 def interaction_matrix(wl, mode: int = ND, modes: Optional[Sequence[int]] = None,
                        wfs: Optional[Sequence[int]] = None, n_threads: int = 0,
-                       affines: Optional[Sequence[Sequence[float]]] = None) -> np.ndarray:
+                       affines: Optional[Sequence[Sequence[float]]] = None,
+                       repair_mask: Optional[np.ndarray] = None,
+                       threshold: float = REPAIR_THRESHOLD) -> np.ndarray:
     """IM of a workload: float64 [rows][n_sel], rows = WFS 0..n-1, each x slopes then y slopes.
 
     ``wfs`` restricts to some sensors (rows of the others are left out);
-    ``affines`` overrides the composite matrices (else composed from ``phys``)."""
+    ``affines`` overrides the composite matrices (else composed from ``phys``);
+    ``repair_mask`` (float32 [ny][nx], source frame) switches the edge repair of PAPER.md:69-76 on
+    (numerical-derivative mode only)."""
     sel = list(range(len(wl.wfs))) if wfs is None else list(wfs)
     blocks = []
     for k in sel:
         w = wl.wfs[k]
         a = compose_affine(w.phys) if affines is None else affines[k]
-        blocks.append(slopes_wfs(wl.cube, w.pupil, w.n_subap, w.n_pix, w.valid, a, w.slope_scale,
-                                 mode, modes, n_threads).T)
+        if repair_mask is not None:
+            assert mode == ND, "edge repair belongs to the numerical-derivative engine"
+            blocks.append(slopes_wfs_repair(wl.cube, repair_mask, w.pupil, w.n_subap, w.n_pix, w.valid, a,
+                                            w.slope_scale, threshold, modes, n_threads).T)
+        else:
+            blocks.append(slopes_wfs(wl.cube, w.pupil, w.n_subap, w.n_pix, w.valid, a, w.slope_scale,
+                                     mode, modes, n_threads).T)
     return np.concatenate(blocks, axis=0)

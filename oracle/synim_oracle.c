@@ -32,6 +32,13 @@
  * pixel valid iff P >= 0.5; for each pixel row of S with first/last valid columns
  * jf < jl: num += phi[row][jl]-phi[row][jf], den += jl-jf; s_x = scale*num/den.
  *
+ * EDGE REPAIR (sec. 2.3 "_repair_interpolated_phase"; readings R18-R22 of DESIGN.md), for modes
+ * that exist only inside a mask given in the SOURCE frame (a DM or pupil mask): see repair_interpolated_phase()
+ * and slopes_nd_core() below.  Pins (tests/test_oracle_repair_pins.py): an all-ones mask changes nothing; a constant
+ * and a linear phase are restored exactly on the ring, so the slopes of a masked tilt are the tilt right up to the
+ * edge; a hand-computed 7x7 example (one valid direction with one reference pixel, two directions of different
+ * kinds); the threshold; an independent restatement with scipy.ndimage.binary_dilation on random masks.
+ *
  * Pins (tests/test_oracle_pins.py): pure tilt -> constant slopes A^T(a,b); quadratic ->
  * linear slopes; identity / integer shift / 90-degree rotations reproduce the input
  * bit for bit; linearity; telescoping identity on full subapertures; equality with
@@ -149,6 +156,81 @@ static void slopes_gtilt(const double *phi, int M, int n_subap, int n_pix, const
 }
 
 /*
+ * Edge repair.  In: phi = the interpolated mode, mu = the mask interpolated through the SAME
+ * composite transform with the same bilinear rule (R18), both on the halo grid (M+2)^2.  Steps, in the paper's order:
+ *   1. strict binarisation and clearing: core = (mu >= threshold), "e.g. 0.999999", compared in
+ *      float64 (R19); phi is set to 0 outside the core;
+ *   2. edge identification: ring = (binary dilation of core) and not core, with the 4-neighbour cross as
+ *      structuring element, one iteration (R20); pixels beyond the halo grid are not core;
+ *   3. omnidirectional extrapolation: for every ring pixel q and each of the four cardinal directions
+ *      d: P1 = q+d, P2 = q+2d ("consecutive reference pixels"); the direction is valid iff P1 is core; its estimate is
+ *      2*phi[P1] - phi[P2] if P2 is core too, else phi[P1]; phi[q] = sum of the estimates / number of valid
+ *      directions (R21).
+ * Out: phi repaired in place (core: unchanged; ring: restored; elsewhere 0), core[] (1/0), ring[] (1/0; may be NULL).
+ */
+static void repair_interpolated_phase(double *phi, const double *mu, int M, double threshold, uint8_t *core, uint8_t *ring)
+{
+    const int P = M + 2;
+    const long n = (long)P * P;
+    for (long q = 0; q < n; ++q) {
+        core[q] = mu[q] >= threshold ? 1 : 0;
+        if (!core[q]) phi[q] = 0.0;
+    }
+    static const int di[4] = {0, 0, 1, -1}, dj[4] = {1, -1, 0, 0};
+    for (int i = 0; i < P; ++i) {
+        for (int j = 0; j < P; ++j) {
+            const long q = (long)i * P + j;
+            if (ring) ring[q] = 0;
+            if (core[q]) continue;
+            double sum = 0.0;
+            int n_dir = 0;
+            for (int d = 0; d < 4; ++d) {
+                const int i1 = i + di[d], j1 = j + dj[d], i2 = i + 2 * di[d], j2 = j + 2 * dj[d];
+                if (i1 < 0 || i1 >= P || j1 < 0 || j1 >= P || !core[(long)i1 * P + j1]) continue;
+                const double p1 = phi[(long)i1 * P + j1];
+                if (i2 >= 0 && i2 < P && j2 >= 0 && j2 < P && core[(long)i2 * P + j2]) sum += 2.0 * p1 - phi[(long)i2 * P + j2];
+                else sum += p1;
+                ++n_dir;
+            }
+            if (n_dir > 0) {          /* q is a 4-neighbour of the core: a ring pixel */
+                if (ring) ring[q] = 1;
+                phi[q] = sum / n_dir;  /* (reads core pixels only, which this loop never writes) */
+            }
+        }
+    }
+}
+
+/* Steps 3-4 after edge repair (R22): central differences of the repaired screen, averaged over the CORE pixels of
+ * the subaperture with the weights P (a pixel outside the core has a stencil that reaches past the ring: no valid
+ * derivative).  A valid subaperture without any weighted core pixel gets slope 0. */
+static void slopes_nd_core(const double *phi, const uint8_t *core, int M, int n_subap, int n_pix, const float *pupil,
+                           const uint8_t *valid, double scale, double *sx, double *sy)
+{
+    const int P = M + 2;
+    int k = 0;
+    for (int a = 0; a < n_subap; ++a) {
+        for (int b = 0; b < n_subap; ++b) {
+            if (!valid[a * n_subap + b]) continue;
+            double w = 0.0, ax = 0.0, ay = 0.0;
+            for (int i = a * n_pix; i < (a + 1) * n_pix; ++i) {
+                for (int j = b * n_pix; j < (b + 1) * n_pix; ++j) {
+                    if (!core[(long)(i + 1) * P + (j + 1)]) continue;
+                    const double p = pupil[(long)i * M + j];
+                    const double dx = (PHI(i, j + 1) - PHI(i, j - 1)) / 2.0;
+                    const double dy = (PHI(i + 1, j) - PHI(i - 1, j)) / 2.0;
+                    w += p;
+                    ax += p * dx;
+                    ay += p * dy;
+                }
+            }
+            sx[k] = w > 0.0 ? scale * ax / w : 0.0;
+            sy[k] = w > 0.0 ? scale * ay / w : 0.0;
+            ++k;
+        }
+    }
+}
+
+/*
  * Slopes of the selected modes for ONE wavefront sensor.
  *   cube      float32 [n_modes_total][ny][nx]
  *   mode_idx  n_sel indices into the cube, or NULL for 0..n_sel-1
@@ -210,6 +292,76 @@ int synim_oracle_wfs(const float *cube, int64_t n_modes_total, const int32_t *mo
         free(phi);
     }
     return err;
+}
+
+/*
+ * Edge-repaired slopes of the selected modes for ONE wavefront sensor: as synim_oracle_wfs in
+ * numerical-derivative mode, with the mode's screen repaired before it is differentiated.
+ *   mask       float32 [ny][nx], the mask of the modes in the SOURCE frame (values in [0, 1])
+ *   threshold  the strict-binarisation threshold (the paper's example: 0.999999)
+ * Returns 0, -1 on bad arguments, -2 on OOM.
+ */
+int synim_oracle_wfs_repair(const float *cube, int64_t n_modes_total, const int32_t *mode_idx, int32_t n_sel,
+                            int32_t ny, int32_t nx, const float *mask, double threshold, const float *pupil,
+                            int32_t n_subap, int32_t n_pix, const uint8_t *valid, const double *a, double scale,
+                            int32_t n_threads, double *out)
+{
+    if (!cube || !mask || !pupil || !valid || !a || !out || ny <= 0 || nx <= 0 || n_subap <= 0 || n_pix <= 0) return -1;
+    const int M = n_subap * n_pix;
+    const size_t np = (size_t)(M + 2) * (size_t)(M + 2);
+    int n_valid = 0;
+    for (int s = 0; s < n_subap * n_subap; ++s) n_valid += valid[s] ? 1 : 0;
+    double *mu = (double *)malloc(sizeof(double) * np);
+    if (!mu) return -2;
+    resample_once(mask, ny, nx, M, a, mu);   /* the mask goes through the same transform, once (R18) */
+    int err = 0;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+    else omp_set_num_threads(omp_get_num_procs());
+#endif
+#pragma omp parallel
+    {
+        double *phi = (double *)malloc(sizeof(double) * np);
+        uint8_t *core = (uint8_t *)malloc(np);
+        if (!phi || !core) {
+#pragma omp atomic write
+            err = -2;
+        }
+#pragma omp for schedule(dynamic, 1)
+        for (int s = 0; s < n_sel; ++s) {
+            if (!phi || !core) continue;
+            const int64_t m = mode_idx ? mode_idx[s] : s;
+            if (m < 0 || m >= n_modes_total) {
+#pragma omp atomic write
+                err = -1;
+                continue;
+            }
+            double *sx = out + (size_t)s * 2 * (size_t)n_valid;
+            resample_once(cube + (size_t)m * (size_t)ny * (size_t)nx, ny, nx, M, a, phi);
+            repair_interpolated_phase(phi, mu, M, threshold, core, NULL);
+            slopes_nd_core(phi, core, M, n_subap, n_pix, pupil, valid, scale, sx, sx + n_valid);
+        }
+        free(phi);
+        free(core);
+    }
+    free(mu);
+    return err;
+}
+
+/* For the pins: the repaired screen of one mode on the halo grid, with its core and ring maps
+ * (all [(M+2)][(M+2)], pixel (i, j) at [(i+1)][(j+1)]). */
+int synim_oracle_repair_screen(const float *g, const float *mask, int32_t ny, int32_t nx, int32_t M, const double *a,
+                               double threshold, double *phi_out, uint8_t *core_out, uint8_t *ring_out)
+{
+    if (!g || !mask || !a || !phi_out || !core_out || !ring_out || M <= 0) return -1;
+    const size_t np = (size_t)(M + 2) * (size_t)(M + 2);
+    double *mu = (double *)malloc(sizeof(double) * np);
+    if (!mu) return -2;
+    resample_once(mask, ny, nx, M, a, mu);
+    resample_once(g, ny, nx, M, a, phi_out);
+    repair_interpolated_phase(phi_out, mu, M, threshold, core_out, ring_out);
+    free(mu);
+    return 0;
 }
 
 /* Steps 1-2 only, for the pins: the resampled screen of one mode, either on the M x M grid

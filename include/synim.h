@@ -55,7 +55,7 @@ typedef enum {
     SYNIM_ERR_UNSUPPORTED_DEVICE = -4, /* current device is not compute capability 10.x */
     SYNIM_ERR_OUT_OF_MEMORY = -5,
     SYNIM_ERR_CUDA = -6,               /* any other CUDA runtime / driver failure */
-    SYNIM_ERR_UNSUPPORTED = -7         /* reserved: a feature not built on this path (none at present) */
+    SYNIM_ERR_UNSUPPORTED = -7         /* a combination that is not built: edge repair with the G-tilt estimator */
 } synim_status;
 
 /* Slope estimator.  ND = finite central differences averaged over the subaperture
@@ -139,6 +139,27 @@ synim_status synim_interaction_matrix(const synim_geometry *geom, const float *d
                                       int32_t bbox_max_h,
                                       const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out,
                                       int64_t ld, void *stream);
+
+/* The same hot path with the paper's EDGE REPAIR (sec. 2.3, "_repair_interpolated_phase"), for modes
+ * that exist only inside a mask given in the SOURCE frame (a DM or pupil mask): their interpolated screen collapses
+ * towards zero along the mask's edge and would corrupt the derivative there.  Per call and sensor (DESIGN.md readings
+ * R18-R22):
+ *   1. d_mask goes through the same composite transform and bilinear rule as the modes (in float64); the strict core
+ *      is mu >= threshold (the paper's example: 0.999999), and the screen is cleared outside it;
+ *   2. the ring is the 4-neighbour dilation of the core minus the core;
+ *   3. a ring pixel becomes the normalised average, over the cardinal directions whose neighbour P1 is core, of
+ *      2*P1 - P2 (P2, the next pixel, core too) or P1;
+ *   then central differences of the repaired screen, averaged over the CORE pixels of each valid subaperture with the
+ *   weights P (a valid subaperture without a weighted core pixel gets slope 0).
+ * Numerical-derivative engine only.  Everything runs on `stream`: three small set-up kernels per sensor, then the fused
+ * kernel (the ring is restored inside it, from extra samples of the staged tile -- the repaired screen is never stored).
+ *   d_mask     DEVICE float32 [ny][nx], values in [0, 1]
+ *   threshold  in (0, 1]
+ * All other arguments, the output layout and the errors as for synim_interaction_matrix. */
+synim_status synim_interaction_matrix_repaired(const synim_geometry *geom, const float *d_influence, int32_t n_modes,
+                                               const int32_t *d_bbox, const int32_t *d_diag, int32_t bbox_max_w,
+                                               int32_t bbox_max_h, const synim_wfs_affine *affine, const float *d_mask,
+                                               double threshold, float *d_out, int64_t ld, void *stream);
 
 /* Tight non-zero extent of every mode of a cube (DEVICE in, DEVICE out int32 [n_modes][4]);
  * an all-zero mode gets (0,0,-1,-1).  d_diag (DEVICE int32 [n_modes][4], or NULL) receives the

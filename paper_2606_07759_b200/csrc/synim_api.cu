@@ -327,11 +327,12 @@ int64_t synim_row_offset(const synim_geometry *g, int32_t w)
 // shared-memory budget of two CTAs per SM; then the tile counts are evened out (68 rows -> 4 x 17, not 16+...+4).
 // Returns false if not even a 1 x 1 tile fits (extreme magnification): the caller falls back to source-space pieces.
 struct TilePlan { int ns, nr, pitch, h; };
-static bool plan_tiles(const synim::WfsDev &d, size_t budget_floats, TilePlan *out)
+static bool plan_tiles(const synim::WfsDev &d, size_t budget_floats, int reach, TilePlan *out)
 {
     const int strip_px = d.spb * d.n_pix, n_strips = (d.n_subap + d.spb - 1) / d.spb;
     auto box = [&](int ns, int nr, int *pitch, int *h) {
-        const double wt = (double)std::min(ns * strip_px, d.M) + 1.0, ht = (double)std::min(nr * d.n_pix, d.M) + 2.0;   // phi pixels - 1 (one more row: look-ahead)
+        // phi pixels - 1 (one more row: look-ahead; reach: what a restored pixel reads beside itself, edge repair)
+        const double wt = (double)std::min(ns * strip_px, d.M) + 1.0 + 2.0 * reach, ht = (double)std::min(nr * d.n_pix, d.M) + 2.0 + 2.0 * reach;
         const double ex = std::fabs(d.fwd[0]) * wt + std::fabs(d.fwd[1]) * ht, ey = std::fabs(d.fwd[3]) * wt + std::fabs(d.fwd[4]) * ht;
         if (!(ex < 1.0e6) || !(ey < 1.0e6)) { *pitch = *h = 1 << 20; return; }
         *pitch = ((int)std::ceil(ex) + 8 + 3) & ~3;   // floor(cmin)-1-slack(<=3) .. floor(cmax)+2
@@ -361,9 +362,14 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
                                            const int32_t *d_origin, int32_t n_modes, const int32_t *d_bbox,
                                            const int32_t *d_diag, int32_t bbox_max_w, int32_t bbox_max_h,
                                            const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out, int64_t ld,
-                                           void *stream)
+                                           void *stream, const float *d_mask = nullptr, double threshold = 0.0)
 {
     if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
+    const bool repair = d_mask != nullptr;
+    if (repair && mode != SYNIM_SLOPES_ND)
+        return fail(SYNIM_ERR_UNSUPPORTED, "edge repair belongs to the numerical-derivative engine (SYNIM_SLOPES_ND)");
+    if (repair && !(threshold > 0.0 && threshold <= 1.0))
+        return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_repaired: threshold %g is not in (0, 1]", threshold);
     if (mode != SYNIM_SLOPES_ND && mode != SYNIM_SLOPES_GTILT) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: unknown slope mode %d", (int)mode);
     if (n_modes == 0) return SYNIM_OK;
     {   // the geometry's buffers live on the device it was created on (an sm_100 one: checked there)
@@ -420,6 +426,42 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         while (d.red_steps < 5 && (1 << d.red_steps) < h.n_pix) ++d.red_steps;
         d.npx_magic = (unsigned)((0x100000000ULL + (unsigned long long)h.n_pix - 1) / (unsigned long long)h.n_pix);   // (unused for 1)
     }
+    // Edge repair: per call and sensor, the mask goes through the sensor's map and becomes pixel
+    // classes, core-restricted weights and a row map that keeps the edge-sum path off anything not core.  The maps
+    // live in ONE stream-ordered allocation, freed (on the stream) after the launches below.
+    struct AsyncBlock {
+        void *p = nullptr; cudaStream_t s = nullptr;
+        ~AsyncBlock() { if (p) cudaFreeAsync(p, s); }
+    } block;
+    const int reach = repair ? synim::kRepairReach : 0;
+    if (repair) {
+        size_t total = 0;
+        std::vector<size_t> off(n_wfs);
+        auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+        for (int w = 0; w < n_wfs; ++w) {
+            const WfsHost &h = g->wfs[w];
+            const size_t np = (size_t)(h.M + 2) * (h.M + 2);
+            off[w] = total;
+            total += up(np) + up(np * sizeof(unsigned short)) + up(sizeof(float) * (size_t)(h.M + synim::kWmapPadRows) * h.M) +
+                     up(sizeof(int) * (size_t)h.n_subap * h.n_subap);
+        }
+        block.s = s;
+        SYNIM_CUDA(cudaMallocAsync(&block.p, total, s));
+        for (int w = 0; w < n_wfs; ++w) {
+            const WfsHost &h = g->wfs[w];
+            const size_t np = (size_t)(h.M + 2) * (h.M + 2);
+            const size_t wbytes = sizeof(float) * (size_t)(h.M + synim::kWmapPadRows) * h.M;
+            char *base = static_cast<char *>(block.p) + off[w];
+            unsigned char *core = reinterpret_cast<unsigned char *>(base);
+            unsigned short *rcode = reinterpret_cast<unsigned short *>(base + up(np));
+            float *wm = reinterpret_cast<float *>(base + up(np) + up(np * sizeof(unsigned short)));
+            int *rows = reinterpret_cast<int *>(base + up(np) + up(np * sizeof(unsigned short)) + up(wbytes));
+            SYNIM_CUDA(cudaMemsetAsync(wm, 0, wbytes, s));   // (the rows of zeros below the map)
+            SYNIM_CUDA(synim::launch_repair_maps(d_mask, ny, nx, dev[w].fwd, threshold, h.n_subap, h.n_pix, h.d_wmap, h.d_subap_row,
+                                                 core, rcode, wm, rows, s));
+            dev[w].wmap = wm; dev[w].subap_row = rows; dev[w].rcode = rcode;
+        }
+    }
     // launch groups: consecutive sensors of one class (subapertures that fit a strip / giant ones), at most
     // kMaxWfsPerLaunch each; a group's rows are contiguous in the column
     std::vector<std::pair<int, int>> groups;   // [first, last) sensor
@@ -436,8 +478,8 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         int off = 0;
         for (int w = gr.first; w < gr.second; ++w) {
             synim::WfsDev &d = dev[w];
-            const double ej = (cap_w + 2) * std::fabs(d.inv[0]) + (cap_h + 2) * std::fabs(d.inv[1]);
-            const double ei = (cap_w + 2) * std::fabs(d.inv[3]) + (cap_h + 2) * std::fabs(d.inv[4]);
+            const double ej = (cap_w + 2) * std::fabs(d.inv[0]) + (cap_h + 2) * std::fabs(d.inv[1]) + 2.0 * reach;
+            const double ei = (cap_w + 2) * std::fabs(d.inv[3]) + (cap_h + 2) * std::fabs(d.inv[4]) + 2.0 * reach;
             auto span = [&](double e) {   // subapertures that floor(x) .. ceil(x + e) can touch
                 const double s_ = std::floor((std::min(e, 1.0e8) + 2.0) / d.n_pix) + 2.0;
                 return (int)std::min<double>(s_, d.n_subap);
@@ -473,6 +515,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         p.cube = d_influence; p.bbox = d_bbox; p.diag = d_diag; p.origin = d_origin; p.out = d_out; p.ld = ld;
         p.n_modes = n_modes; p.ny = ny; p.nx = nx; p.n_wfs = nw;
         p.addr_bias = 0x4B400000u << 2;
+        p.reach = reach;
         for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
         if (dense && dev[w0].spb > 0) {
             // two CTAs per SM: half the SM's shared memory less the per-CTA reserve and the static part
@@ -481,7 +524,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
             int tiles = 0, box_floats = 0, tab = 0;
             for (int w = 0; w < nw && fits; ++w) {
                 TilePlan tp;
-                fits = plan_tiles(p.wfs[w], budget / sizeof(float), &tp);
+                fits = plan_tiles(p.wfs[w], budget / sizeof(float), reach, &tp);
                 if (!fits) break;
                 synim::WfsDev &d = p.wfs[w];
                 d.tile_ns = tp.ns; d.tile_nr = tp.nr; d.box_pitch = tp.pitch; d.box_h = tp.h;
@@ -521,7 +564,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
                             std::memcpy(maps.m[w], &tm, sizeof(tm));
                         }
                     }
-                    SYNIM_CUDA(synim::launch_tiles(q, maps, tsmem, mode == SYNIM_SLOPES_GTILT, s));
+                    SYNIM_CUDA(synim::launch_tiles(q, maps, tsmem, mode == SYNIM_SLOPES_GTILT, repair, s));
                 }
                 continue;
             }
@@ -543,7 +586,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
             const WfsHost &last = g->wfs[w0 + nw - 1];
             p.zero_count = last.row_x + 2 * last.n_valid - p.zero_begin;
         }
-        SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, mode == SYNIM_SLOPES_GTILT, s));
+        SYNIM_CUDA(synim::launch_strip(p, &tmap, smem, mode == SYNIM_SLOPES_GTILT, repair, s));
     }
     return SYNIM_OK;
 }
@@ -556,6 +599,17 @@ synim_status synim_interaction_matrix(const synim_geometry *g, const float *d_in
     if (!g) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
     return run_interaction_matrix(g, d_influence, g->ny, g->nx, nullptr, n_modes, d_bbox, d_diag, bbox_max_w, bbox_max_h, affine,
                                   mode, d_out, ld, stream);
+}
+
+synim_status synim_interaction_matrix_repaired(const synim_geometry *g, const float *d_influence, int32_t n_modes,
+                                               const int32_t *d_bbox, const int32_t *d_diag, int32_t bbox_max_w, int32_t bbox_max_h,
+                                               const synim_wfs_affine *affine, const float *d_mask, double threshold, float *d_out,
+                                               int64_t ld, void *stream)
+{
+    if (!g) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_repaired: NULL geometry");
+    if (!d_mask) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_repaired: NULL mask");
+    return run_interaction_matrix(g, d_influence, g->ny, g->nx, nullptr, n_modes, d_bbox, d_diag, bbox_max_w, bbox_max_h, affine,
+                                  SYNIM_SLOPES_ND, d_out, ld, stream, d_mask, threshold);
 }
 
 synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx, int32_t *d_bbox,

@@ -11,6 +11,11 @@ constexpr int kWmapPadRows = 8;        // rows of zeros below each sensor's weig
 constexpr int kSubapGeneral = 1 << 30; // flag in a row-map entry: valid subaperture whose pixel weights differ
 constexpr int kSubapRowMask = kSubapGeneral - 1;
 constexpr int kStripMaxCols = 30;      // D columns of a strip (one per lane, plus a halo lane on either side)
+// edge repair: class of a pixel of the interpolated screen.  Bit 0: the pixel belongs to the strict
+// core.  Otherwise bits 1..4 say in which of the directions +x, -x, +y, -y the neighbour P1 is a core pixel (any of
+// them set: a ring pixel), bits 5..8 whether the next pixel P2 in that direction is one too.
+constexpr int kRepairCore = 1, kRepairP1Shift = 1, kRepairP2Shift = 5, kRepairRingMask = 0x1e;
+constexpr int kRepairReach = 2;        // a restored pixel reads up to two pixels away
 
 // One sensor as the kernel sees it.  All coordinates are ABSOLUTE pixel indices: WFS pixel (i, j)
 // (row, column) samples the source grid at
@@ -25,6 +30,8 @@ struct WfsDev {
     const float *gx, *gy;    // [M][M]  G-tilt coefficients (gtilt_maps_kernel); same rows of zeros below
     const int *subap_row;    // [n_subap^2] index among the valid subapertures (| kSubapGeneral if its pixel weights
                              // differ), -1 if invalid
+    const unsigned short *rcode;   // edge repair only: [(M+2)][(M+2)] class of every pixel of the halo grid -1..M
+                                   // (kRepair* bits below), built per call by repair_maps
     float scale;             // slope_scale
     float w_uniform;         // 0.5 / n_pix^2: the weight of every pixel of a uniform subaperture
     int M, n_subap, n_pix;
@@ -57,6 +64,7 @@ struct ImParams {
     unsigned addr_bias;         // (bits of 1.5*2^23) << 2 mod 2^32, see process_strip
     int tab_floats;             // size of the CTA's slope table (multiple of 4)
     int tiles_total;            // tile kernel: tiles of one mode over all sensors of the launch
+    int reach;                  // extra pixels around a tile / a footprint that a sample may touch: 0, or kRepairReach
     WfsDev wfs[kMaxWfsPerLaunch];
 };
 
@@ -69,10 +77,20 @@ struct alignas(64) TileMaps {
 // launchers; all asynchronous on `stream`, return the launch status.
 // The hot path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
 // {patch_pitch, patch_h, 1}
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream);
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, bool repair,
+                         cudaStream_t stream);
 // Dense modes over sensors whose subapertures fit a strip: one CTA per (mode, sensor, tile of the WFS grid);
 // maps.m[w] is sensor w's CUtensorMap over the cube with box {box_pitch, box_h, 1}
-cudaError_t launch_tiles(const ImParams &p, const TileMaps &maps, size_t smem_bytes, bool gtilt, cudaStream_t stream);
+cudaError_t launch_tiles(const ImParams &p, const TileMaps &maps, size_t smem_bytes, bool gtilt, bool repair,
+                         cudaStream_t stream);
+// Edge repair, per call and sensor: the mask [ny][nx] is interpolated through the sensor's map fwd
+// (float64), thresholded into the strict core, and turned into (a) the pixel classes rcode [(M+2)^2], (b) the
+// reduction weights wmap_out = 0.5*P*core / sum_S(P*core) (from wmap_in = 0.5*P/W_S), (c) the row map rows_out =
+// rows_in with kSubapGeneral set unless the subaperture and the pixels its edge sums read are all core.
+// core is scratch: (M+2)^2 bytes.
+cudaError_t launch_repair_maps(const float *d_mask, int ny, int nx, const double *fwd, double threshold, int n_subap, int n_pix,
+                               const float *wmap_in, const int *rows_in, unsigned char *core, unsigned short *rcode,
+                               float *wmap_out, int *rows_out, cudaStream_t stream);
 cudaError_t launch_subap_weights(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix,
                                  float *d_wmap, int *d_subap_row, int *d_error_flag, cudaStream_t stream);
 cudaError_t launch_gtilt_maps(const float *d_pupil, const uint8_t *d_valid, int n_subap, int n_pix, float *d_gx, float *d_gy,

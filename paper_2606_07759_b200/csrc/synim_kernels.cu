@@ -103,6 +103,109 @@ __global__ void __launch_bounds__(128) gtilt_maps_kernel(const float *__restrict
     }
 }
 
+// ---- edge repair, per call (readings R18-R22) -----------------------------------------
+// Step 1, the strict core: the mask goes through the SAME map and the same bilinear rule as the modes (zero outside
+// the grid), in float64 -- float32 coordinates could not tell a weight of 1e-6 from 0 -- and core = (mu >= threshold).
+struct Fwd6 { double a[6]; };
+__global__ void __launch_bounds__(256) repair_core_kernel(const float *__restrict__ mask, int ny, int nx, Fwd6 f, double threshold,
+                                                          int M, unsigned char *__restrict__ core)
+{
+    const int P = M + 2;
+    const int q = blockIdx.x * 256 + threadIdx.x;
+    if (q >= P * P) return;
+    const int i = q / P - 1, j = q - (i + 1) * P - 1;
+    const double col = f.a[0] * (double)j + f.a[1] * (double)i + f.a[2];
+    const double row = f.a[3] * (double)j + f.a[4] * (double)i + f.a[5];
+    const double fc = floor(col), fr = floor(row);
+    double v00 = 0.0, v01 = 0.0, v10 = 0.0, v11 = 0.0;
+    if (fc >= -1.0 && fc <= (double)nx && fr >= -1.0 && fr <= (double)ny) {
+        const int c0 = (int)fc, r0 = (int)fr;
+        const bool cl = c0 >= 0 && c0 < nx, ch = c0 + 1 >= 0 && c0 + 1 < nx;
+        if (r0 >= 0 && r0 < ny) {
+            if (cl) v00 = (double)__ldg(mask + (size_t)r0 * nx + c0);
+            if (ch) v01 = (double)__ldg(mask + (size_t)r0 * nx + c0 + 1);
+        }
+        if (r0 + 1 >= 0 && r0 + 1 < ny) {
+            if (cl) v10 = (double)__ldg(mask + (size_t)(r0 + 1) * nx + c0);
+            if (ch) v11 = (double)__ldg(mask + (size_t)(r0 + 1) * nx + c0 + 1);
+        }
+    }
+    const double fx = col - fc, fy = row - fr;
+    const double mu = (1.0 - fy) * ((1.0 - fx) * v00 + fx * v01) + fy * ((1.0 - fx) * v10 + fx * v11);
+    core[q] = mu >= threshold ? 1 : 0;
+}
+
+// Steps 2-3 as pixel classes: the ring is the 4-neighbour dilation of the core minus the core, and a ring pixel's
+// restored value averages, over the directions whose P1 is core, 2*phi[P1] - phi[P2] (P2 core) or phi[P1].  Pixels
+// beyond the halo grid are not core.
+__global__ void __launch_bounds__(256) repair_code_kernel(const unsigned char *__restrict__ core, int M, unsigned short *__restrict__ code)
+{
+    const int P = M + 2;
+    const int q = blockIdx.x * 256 + threadIdx.x;
+    if (q >= P * P) return;
+    const int i = q / P, j = q - i * P;
+    if (core[q]) { code[q] = (unsigned short)kRepairCore; return; }
+    const int di[4] = {0, 0, 1, -1}, dj[4] = {1, -1, 0, 0};
+    int c = 0;
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+        const int i1 = i + di[d], j1 = j + dj[d], i2 = i + 2 * di[d], j2 = j + 2 * dj[d];
+        if (i1 < 0 || i1 >= P || j1 < 0 || j1 >= P || !core[i1 * P + j1]) continue;
+        c |= 1 << (kRepairP1Shift + d);
+        if (i2 >= 0 && i2 < P && j2 >= 0 && j2 < P && core[i2 * P + j2]) c |= 1 << (kRepairP2Shift + d);
+    }
+    code[q] = (unsigned short)c;
+}
+
+// The reduction weights over the core (R22) and the subapertures that may keep the edge-sum path: one CTA per
+// subaperture.  wmap_in = 0.5*P/W_S, so 0.5*P*core / sum_S(P*core) = 0.5 * wmap_in*core / sum_S(wmap_in*core).
+__global__ void __launch_bounds__(128) repair_weights_kernel(const unsigned char *__restrict__ core, int n_subap, int n_pix,
+                                                             const float *__restrict__ wmap_in, const int *__restrict__ rows_in,
+                                                             float *__restrict__ wmap_out, int *__restrict__ rows_out)
+{
+    __shared__ double part[4];
+    __shared__ int bad[4];
+    const int s = blockIdx.x, a = s / n_subap, b = s - a * n_subap;
+    const int M = n_subap * n_pix, P = M + 2, n = n_pix * n_pix;
+    const int row_in = rows_in[s];
+    double acc = 0.0;
+    int notcore = 0;
+    for (int e = threadIdx.x; e < n; e += 128) {
+        const int r = e / n_pix, c = e - r * n_pix;
+        const int i = a * n_pix + r, j = b * n_pix + c;
+        const bool co = core[(i + 1) * P + (j + 1)] != 0;
+        if (co) acc += (double)wmap_in[(size_t)i * M + j];
+        notcore |= !co;
+    }
+    // the pixels the edge sums read beside the subaperture: one row above and below, one column left and right
+    for (int e = threadIdx.x; e < 4 * n_pix; e += 128) {
+        const int side = e / n_pix, t = e - side * n_pix;
+        const int i = side == 0 ? a * n_pix - 1 : (side == 1 ? (a + 1) * n_pix : a * n_pix + t);
+        const int j = side == 2 ? b * n_pix - 1 : (side == 3 ? (b + 1) * n_pix : b * n_pix + t);
+        notcore |= core[(i + 1) * P + (j + 1)] == 0;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        notcore |= __shfl_xor_sync(0xffffffffu, notcore, o);
+    }
+    if ((threadIdx.x & 31) == 0) { part[threadIdx.x >> 5] = acc; bad[threadIdx.x >> 5] = notcore; }
+    __syncthreads();
+    const double total = part[0] + part[1] + part[2] + part[3];
+    if (threadIdx.x == 0) {
+        int r = row_in;
+        if (r >= 0 && (bad[0] | bad[1] | bad[2] | bad[3])) r |= kSubapGeneral;
+        rows_out[s] = r;
+    }
+    const bool ok = row_in >= 0 && total > 0.0;
+    for (int e = threadIdx.x; e < n; e += 128) {
+        const int r = e / n_pix, c = e - r * n_pix;
+        const int i = a * n_pix + r, j = b * n_pix + c;
+        const size_t at = (size_t)i * M + j;
+        const bool co = core[(i + 1) * P + (j + 1)] != 0;
+        wmap_out[at] = (ok && co) ? (float)(0.5 * (double)wmap_in[at] / total) : 0.0f;
+    }
+}
+
 // one CTA per mode: tight non-zero extent (x0,y0,x1,y1) and, if asked for, the diagonal extents
 // (min x+y, max x+y, min x-y, max x-y) of the non-zero pixels: together the support's bounding octagon
 __global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ cube, int ny, int nx,
@@ -200,6 +303,26 @@ cudaError_t launch_compute_bboxes(const float *d_cube, int n_modes, int ny, int 
     if (n_modes <= 0) return cudaSuccess;
     note_launch();
     bbox_kernel<<<n_modes, 256, 0, stream>>>(d_cube, ny, nx, d_bbox, d_diag);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_repair_maps(const float *d_mask, int ny, int nx, const double *fwd, double threshold, int n_subap, int n_pix,
+                               const float *wmap_in, const int *rows_in, unsigned char *core, unsigned short *rcode,
+                               float *wmap_out, int *rows_out, cudaStream_t stream)
+{
+    const int M = n_subap * n_pix, np = (M + 2) * (M + 2);
+    Fwd6 f;
+    for (int k = 0; k < 6; ++k) f.a[k] = fwd[k];
+    note_launch();
+    repair_core_kernel<<<(np + 255) / 256, 256, 0, stream>>>(d_mask, ny, nx, f, threshold, M, core);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    note_launch();
+    repair_code_kernel<<<(np + 255) / 256, 256, 0, stream>>>(core, M, rcode);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    note_launch();
+    repair_weights_kernel<<<n_subap * n_subap, 128, 0, stream>>>(core, n_subap, n_pix, wmap_in, rows_in, wmap_out, rows_out);
     return cudaGetLastError();
 }
 

@@ -227,12 +227,18 @@ __device__ __forceinline__ int div_npx(int x, int npx, unsigned magic) { return 
 // pruning; (b) coordinates are taken relative to the pre-image of the strip's own centre (an integer source pixel
 // folded into the address base), which keeps |col|, |row| below ~64 and their float32 spacing below 4e-6 pixels
 // however large the box is; (c) a unit none of whose subapertures is valid is SKIPPED (nothing is sampled for it).
-template <bool kGtilt, bool kAligned, bool kTile>
+// kRepair (edge repair; numerical derivative only): the stencil reads the REPAIRED screen -- phi on
+// the strict core, the normalised average of 2*P1-P2 / P1 over the valid cardinal directions on the ring (each P a
+// bilinear sample of its own, taken by the lane that needs it), 0 elsewhere -- per the pixel classes W.rcode that
+// repair_maps built for this call; W.wmap then holds 0.5*P*core/sum(P*core) and W.subap_row flags as general every
+// subaperture that is not core throughout, so the edge-sum path only ever sees unrepaired pixels.
+template <bool kGtilt, bool kAligned, bool kTile, bool kRepair>
 __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
                                               uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp,
                                               uint32_t scr = 0u)
 {
     static_assert(!kTile || kAligned, "tiles are made of aligned strips");
+    static_assert(!kRepair || !kGtilt, "edge repair belongs to the numerical-derivative engine");
     constexpr bool kEdge = kAligned && !kGtilt && SYNIM_EDGE_SUM != 0;   // the edge-sum path exists
     constexpr int kRows = kStripRows;
     static_assert(kRows == 2, "the segment loops are written for two rows per iteration");
@@ -269,8 +275,11 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // phi rows whose pixel segment [lane 0 .. lane nC+1] can reach the support's octagon (a sample is
     // non-zero only if 0 <= col < cw, 0 <= row < ch and inside the diagonal limits); every sample of a
     // row lies between its two end points, and each limit is a half-plane
-    const float bcL = __shfl_sync(kFull, bc, 0), brL = __shfl_sync(kFull, br, 0);
-    const float bcR = __shfl_sync(kFull, bc, nC + 1), brR = __shfl_sync(kFull, br, nC + 1);
+    // (kRepair: a restored pixel reads up to kRepairReach pixels away, along its row or its column)
+    const float a0f = (float)W.fwd[0], a3f = (float)W.fwd[3];
+    const float reachf = kRepair ? (float)kRepairReach : 0.0f;
+    const float bcL = __shfl_sync(kFull, bc, 0) - reachf * a0f, brL = __shfl_sync(kFull, br, 0) - reachf * a3f;
+    const float bcR = __shfl_sync(kFull, bc, nC + 1) + reachf * a0f, brR = __shfl_sync(kFull, br, nC + 1) + reachf * a3f;
     int first = 0x7fffffff, last = -1;
     if (kTile) { first = 0; last = nR + 1; }
     for (int g = 0; !kTile && g < nR + 2; g += 32) {
@@ -289,7 +298,8 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         }
     }
     if (last < 0) return;
-    const int d_lo = max(first - 1, 1), d_hi = min(last + 1, nR);   // D rows that can be non-zero
+    const int row_reach = kRepair ? 1 + kRepairReach : 1;
+    const int d_lo = max(first - row_reach, 1), d_hi = min(last + row_reach, nR);   // D rows that can be non-zero
     if (d_hi < d_lo) return;
 
     // segments of lanes that belong to one subaperture column
@@ -391,8 +401,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     const uint32_t cw_bits = __float_as_uint(cwf), ch_bits = __float_as_uint(chf);
     const float pitchf = cb.pitchf;
     const uint32_t rpitch4 = (uint32_t)cb.pitch * 4u;
-    auto sample = [&](float rf) -> float {
-        const float col = fmaf(a1, rf, bc), row = fmaf(a4, rf, br);
+    auto sample_xy = [&](float col, float row) -> float {
         const float tc = __fadd_rd(col, kMagicFloor), tr = __fadd_rd(row, kMagicFloor);   // magic + floor
         const float fx = col - (tc - kMagicFloor), fy = row - (tr - kMagicFloor);
         // magic + c0 + r0*pitch is exact: its mantissa is the element index (a negative index borrows from
@@ -433,6 +442,37 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
               "r"(rpitch4));
         return phi;
     };
+    auto sample = [&](float rf) -> float { return sample_xy(fmaf(a1, rf, bc), fmaf(a4, rf, br)); };
+    // the repaired screen (kRepair) at phi row rr (counted from i0-1; rf is its float, re-based) of this lane's column
+    const int jhalo = (kTile ? min(jcol, jA + nC) : jcol) + 1;   // column on the halo grid, >= 0
+    auto sample_r = [&](float rf, int rr) -> float {
+        float v = sample(rf);
+        if (kRepair) {
+            const int irow = i0 + rr;   // row on the halo grid (absolute row i0-1+rr, plus one)
+            int code = 0;
+            if (irow <= W.M + 1 && jhalo <= W.M + 1) code = (int)__ldg(W.rcode + (size_t)irow * (size_t)(W.M + 2) + jhalo);
+            if (!(code & kRepairCore)) {
+                v = 0.0f;                              // cleared outside the strict core
+                if (code & kRepairRingMask) {          // ring: restored from the core
+                    float acc = 0.0f, cnt = 0.0f;
+#pragma unroll 1
+                    for (int dir = 0; dir < 4; ++dir) {   // +x, -x, +y, -y (rare: one copy of the code is enough)
+                        if (!((code >> (kRepairP1Shift + dir)) & 1)) continue;
+                        const float sgn = (dir & 1) ? -1.0f : 1.0f;
+                        const float dj = dir < 2 ? sgn : 0.0f, di = dir < 2 ? 0.0f : sgn;
+                        const float p1 = sample_xy(fmaf(a1, rf + di, fmaf(a0f, dj, bc)), fmaf(a4, rf + di, fmaf(a3f, dj, br)));
+                        float est = p1;
+                        if ((code >> (kRepairP2Shift + dir)) & 1)
+                            est = 2.0f * p1 - sample_xy(fmaf(a1, rf + 2.0f * di, fmaf(a0f, 2.0f * dj, bc)),
+                                                        fmaf(a4, rf + 2.0f * di, fmaf(a3f, 2.0f * dj, br)));
+                        acc += est; cnt += 1.0f;
+                    }
+                    v = acc / cnt;
+                }
+            }
+        }
+        return v;
+    };
 #ifdef SYNIM_CHECKS
     const uint32_t wlimit = (uint32_t)(M + kWmapPadRows) * (uint32_t)M;
 #define SYNIM_WCHECK(o) do { if ((o) >= wlimit) __trap(); } while (0)
@@ -462,7 +502,9 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         const int rebase_rows = kRebaseUnits * npx;
         if (kTile) rebase(d - 1, min(d_end, d - 1 + rebase_rows) + 1);
         float rf = (float)(d + 1 - roff);
-        float pmA = sample((float)(d - 1 - roff)), pmB = sample((float)(d - roff));   // phi[d-1], phi[d]
+        float pmA, pmB;   // phi[d-1], phi[d]
+        if (kRepair && gen) { pmA = sample_r((float)(d - 1 - roff), d - 1); pmB = sample_r((float)(d - roff), d); }
+        else { pmA = sample((float)(d - 1 - roff)); pmB = sample((float)(d - roff)); }
         if (gen) {
             const float *wm = kGtilt ? W.gx : W.wmap, *wm2 = kGtilt ? W.gy : W.wmap;
             // weight map offsets (elements).  The map has kWmapPadRows rows of zeros below row M-1: halo lanes
@@ -487,7 +529,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
                 }
                 float cur[kRows];   // phi[d+1 .. d+kRows]
 #pragma unroll
-                for (int k = 0; k < kRows; ++k) cur[k] = sample(rf + (float)k);
+                for (int k = 0; k < kRows; ++k) cur[k] = kRepair ? sample_r(rf + (float)k, d + 1 + k) : sample(rf + (float)k);
                 rf += (float)kRows;
                 // D rows d, d+1: D_y from registers, D_x from the neighbouring lanes.  A row past d_hi has D = 0
                 // exactly (or a weight from the rows of zeros); a row past d_end is the next segment's.
@@ -644,8 +686,9 @@ __device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, 
             vertex(xa, Y); vertex(xb, Y);
         }
         const double lim = 1.0e9;
-        r_j0 = max(0, (int)floor(fmax(jmin, -lim))); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)));
-        r_i0 = max(0, (int)floor(fmax(imin, -lim))); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)));
+        // (p.reach: with edge repair a restored pixel carries phi up to kRepairReach pixels further)
+        r_j0 = max(0, (int)floor(fmax(jmin, -lim)) - p.reach); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)) + p.reach);
+        r_i0 = max(0, (int)floor(fmax(imin, -lim)) - p.reach); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)) + p.reach);
         int4 win = make_int4(0, 0, 0, 0);
         if (r_j1 >= r_j0 && r_i1 >= r_i0) {
             r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
@@ -661,7 +704,7 @@ __device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, 
 // All warps, after a barrier: fetch the IM rows of the windows' subapertures (needed only when the table
 // is stored: asynchronously, so that the store at the end waits for nothing), then sample the strips of
 // every sensor's footprint.
-template <bool kGtilt, bool kAligned>
+template <bool kGtilt, bool kAligned, bool kRepair>
 __device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, int lane, const int4 *s_box, const int4 *s_win,
                                                   int *s_next_ptr, const CellBox &cb, uint32_t tab_base, uint32_t krow_base,
                                                   ZeroPacer &zp)
@@ -713,10 +756,10 @@ __device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, i
         const uint32_t tab = tab_base + (uint32_t)W.tab_off * 4u;
         if (kAligned) {
             const int bA = b0 + (t - base) * spb;
-            process_strip<kGtilt, true, false>(W, i0, i1, bA * W.n_pix, min(spb, b0 + nb - bA) * W.n_pix, cb, p.addr_bias, tab, a0, b0, nb, zp);
+            process_strip<kGtilt, true, false, kRepair>(W, i0, i1, bA * W.n_pix, min(spb, b0 + nb - bA) * W.n_pix, cb, p.addr_bias, tab, a0, b0, nb, zp);
         } else {
             const int jA = j0 + (t - base) * kStripCols;
-            process_strip<kGtilt, false, false>(W, i0, i1, jA, min(kStripCols, j1 - jA + 1), cb, p.addr_bias, tab, a0, b0, nb, zp);
+            process_strip<kGtilt, false, false, kRepair>(W, i0, i1, jA, min(kStripCols, j1 - jA + 1), cb, p.addr_bias, tab, a0, b0, nb, zp);
         }
     }
 }
@@ -749,8 +792,8 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
     }
 }
 
-template <bool kGtilt, bool kAligned>
-__global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
+template <bool kGtilt, bool kAligned, bool kRepair>
+__global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
                                                                                      const __grid_constant__ CUtensorMap tmap)
 {
     // [ TMA box: patch_pitch x patch_h floats | table: tab_floats | rows: tab_floats / 2 ints ]
@@ -848,7 +891,7 @@ __global__ void __launch_bounds__(kStripThreads, SYNIM_STRIP_MINB) synim_strip_k
             }
             bar_sync(1, kComputeThreads);   // footprints (and a cleared ring) visible
 
-            sample_footprints<kGtilt, kAligned>(p, warp, lane, s_box, s_win, &s_next, cb, tab_base, krow_base, zp);
+            sample_footprints<kGtilt, kAligned, kRepair>(p, warp, lane, s_box, s_win, &s_next, cb, tab_base, krow_base, zp);
             if (multi) {
                 cp_async_wait_all();
                 bar_sync(1, kComputeThreads);   // every warp is done with this box and this piece's table
@@ -895,7 +938,7 @@ __device__ __forceinline__ void tma_load_box_plain(void *dst, const void *map, u
 }
 
 // grid: x = tile of the mode (all sensors of the launch), y = mode -- the tiles of a mode are neighbours in launch order
-template <bool kGtilt>
+template <bool kGtilt, bool kRepair>
 __global__ void __launch_bounds__(kTileThreads, 2) synim_tile_kernel(const __grid_constant__ ImParams p,
                                                                      const __grid_constant__ TileMaps maps)
 {
@@ -930,8 +973,9 @@ __global__ void __launch_bounds__(kTileThreads, 2) synim_tile_kernel(const __gri
     if (!__syncthreads_or(any)) return;
 
     // pre-image of the tile's phi pixels (halo included): bounding box of the four corners, float64
-    const double jl = (double)(b0 * npx - 1), jh = (double)((b0 + nb) * npx);
-    const double il = (double)(a0 * npx - 1), ih = (double)((a0 + na) * npx + 1);   // (+1: the general path's row look-ahead)
+    // (+1 below: the general path's row look-ahead; p.reach: what a restored pixel reads beside itself)
+    const double jl = (double)(b0 * npx - 1 - p.reach), jh = (double)((b0 + nb) * npx + p.reach);
+    const double il = (double)(a0 * npx - 1 - p.reach), ih = (double)((a0 + na) * npx + 1 + p.reach);
     const double cmin = W.fwd[2] + fmin(W.fwd[0] * jl, W.fwd[0] * jh) + fmin(W.fwd[1] * il, W.fwd[1] * ih);
     const double rmin = W.fwd[5] + fmin(W.fwd[3] * jl, W.fwd[3] * jh) + fmin(W.fwd[4] * il, W.fwd[4] * ih);
     const double lim = 1.0e9;
@@ -971,7 +1015,7 @@ __global__ void __launch_bounds__(kTileThreads, 2) synim_tile_kernel(const __gri
         if (it >= total) break;
         const int c = it / ns, sidx = it - c * ns;
         const int bA = b0 + sidx * spb, aA = a0 + c * cr, aE = min(aA + cr, a0 + na);
-        process_strip<kGtilt, true, true>(W, aA * npx, aE * npx - 1, bA * npx, min(spb, b0 + nb - bA) * npx, cb, p.addr_bias,
+        process_strip<kGtilt, true, true, kRepair>(W, aA * npx, aE * npx - 1, bA * npx, min(spb, b0 + nb - bA) * npx, cb, p.addr_bias,
                                           tab_base, a0, b0, nb, zp, scr);
     }
     __syncthreads();   // table complete
@@ -991,21 +1035,23 @@ __global__ void __launch_bounds__(kTileThreads, 2) synim_tile_kernel(const __gri
 
 }  // namespace
 
-cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, cudaStream_t stream)
+cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, bool repair, cudaStream_t stream)
 {
     if (p.n_modes <= 0) return cudaSuccess;
+    if (gtilt && repair) return cudaErrorInvalidValue;
     bool aligned = true;   // one class of sensors per launch (the host groups them)
     for (int w = 0; w < p.n_wfs; ++w) aligned = aligned && p.wfs[w].spb > 0;
     for (int w = 0; w < p.n_wfs; ++w)
         if (!aligned && p.wfs[w].spb > 0) return cudaErrorInvalidValue;
-    auto kernel = gtilt ? (aligned ? synim_strip_kernel<true, true> : synim_strip_kernel<true, false>)
-                        : (aligned ? synim_strip_kernel<false, true> : synim_strip_kernel<false, false>);
+    auto kernel = repair ? (aligned ? synim_strip_kernel<false, true, true> : synim_strip_kernel<false, false, true>)
+                  : gtilt ? (aligned ? synim_strip_kernel<true, true, false> : synim_strip_kernel<true, false, false>)
+                          : (aligned ? synim_strip_kernel<false, true, false> : synim_strip_kernel<false, false, false>);
     // the opt-in shared-memory limit only ever has to grow (per device; a race sets it twice, harmlessly)
-    static size_t granted[4][64] = {};
+    static size_t granted[6][64] = {};
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    size_t &have = granted[(gtilt ? 2 : 0) + (aligned ? 1 : 0)][dev & 63];
+    size_t &have = granted[(repair ? 4 : (gtilt ? 2 : 0)) + (aligned ? 1 : 0)][dev & 63];
     if (smem_bytes > have) {
         e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return e;
@@ -1018,19 +1064,20 @@ cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_
     return cudaGetLastError();
 }
 
-cudaError_t launch_tiles(const ImParams &p, const TileMaps &maps, size_t smem_bytes, bool gtilt, cudaStream_t stream)
+cudaError_t launch_tiles(const ImParams &p, const TileMaps &maps, size_t smem_bytes, bool gtilt, bool repair, cudaStream_t stream)
 {
+    if (gtilt && repair) return cudaErrorInvalidValue;
     if (p.n_modes <= 0 || p.tiles_total <= 0) return cudaSuccess;
     for (int w = 0; w < p.n_wfs; ++w)
         if (p.wfs[w].spb <= 0) return cudaErrorInvalidValue;
     if (p.n_modes > 65535) return cudaErrorInvalidValue;   // (the host splits larger batches)
-    auto kernel = gtilt ? synim_tile_kernel<true> : synim_tile_kernel<false>;
-    static size_t granted[2][64] = {};
+    auto kernel = repair ? synim_tile_kernel<false, true> : (gtilt ? synim_tile_kernel<true, false> : synim_tile_kernel<false, false>);
+    static size_t granted[3][64] = {};
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     smem_bytes += sizeof(float) * (size_t)(kTileWarps * kTileScratchFloats);
-    size_t &have = granted[gtilt ? 1 : 0][dev & 63];
+    size_t &have = granted[repair ? 2 : (gtilt ? 1 : 0)][dev & 63];
     if (smem_bytes > have) {
         e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return e;

@@ -21,7 +21,8 @@ SLOPES_ND, SLOPES_GTILT = 0, 1
 
 #: every symbol include/synim.h declares
 EXPORTS = ("synim_compose_affine", "synim_create_geometry", "synim_num_rows", "synim_num_valid",
-           "synim_row_offset", "synim_interaction_matrix", "synim_compute_bboxes", "synim_bbox_extent",
+           "synim_row_offset", "synim_interaction_matrix", "synim_interaction_matrix_repaired", "synim_compute_bboxes",
+           "synim_bbox_extent",
            "synim_interaction_matrix_host", "synim_destroy", "synim_last_error", "synim_version",
            "synim_launch_count")
 
@@ -75,6 +76,9 @@ def lib() -> ctypes.CDLL:
         L.synim_interaction_matrix.restype = ctypes.c_int
         L.synim_interaction_matrix.argtypes = [vp, vp, i32, vp, vp, i32, i32, ctypes.POINTER(WfsAffine), ctypes.c_int,
                                                vp, i64, vp]
+        L.synim_interaction_matrix_repaired.restype = ctypes.c_int
+        L.synim_interaction_matrix_repaired.argtypes = [vp, vp, i32, vp, vp, i32, i32, ctypes.POINTER(WfsAffine), vp,
+                                                        ctypes.c_double, vp, i64, vp]
         L.synim_compute_bboxes.restype = ctypes.c_int
         L.synim_compute_bboxes.argtypes = [vp, i32, i32, i32, vp, vp, vp]
         L.synim_bbox_extent.restype = ctypes.c_int
@@ -234,11 +238,16 @@ def bbox_extent(bbox, stream=None):
     return int(w.value), int(h.value)
 
 
+REPAIR_THRESHOLD = 0.999999   #: the paper's example value for the strict binarisation
+
+
 def interaction_matrix(geom: Geometry, cube, bbox, affines: Sequence[Sequence[float]],
                        scales: Optional[Sequence[float]] = None, out=None, bbox_max=(0, 0),
-                       mode: int = SLOPES_ND, stream=None, diag=None):
+                       mode: int = SLOPES_ND, stream=None, diag=None, repair_mask=None,
+                       threshold: float = REPAIR_THRESHOLD):
     """synim_interaction_matrix on CUDA tensors.  Returns ``out`` viewed as [n_modes][ld] (row k of the
-    view is IM column k: the buffer is the column-major IM)."""
+    view is IM column k: the buffer is the column-major IM).  With ``repair_mask`` (CUDA float32 [ny][nx], the
+    modes' mask in the source frame) the call is synim_interaction_matrix_repaired (edge repair)."""
     import torch
     assert cube.is_cuda and cube.dtype == torch.float32 and cube.is_contiguous() and cube.dim() == 3
     n = int(cube.shape[0])
@@ -261,6 +270,15 @@ def interaction_matrix(geom: Geometry, cube, bbox, affines: Sequence[Sequence[fl
         assert diag.is_cuda and diag.dtype == torch.int32 and diag.is_contiguous() and tuple(diag.shape) == (n, 4)
         dptr = diag.data_ptr()
     arr = _affine_array(affines, scales)
+    if repair_mask is not None:
+        assert repair_mask.is_cuda and repair_mask.dtype == torch.float32 and repair_mask.is_contiguous()
+        assert tuple(repair_mask.shape) == (geom.ny, geom.nx)
+        if mode != SLOPES_ND:
+            raise ValueError("edge repair belongs to the numerical-derivative engine")
+        _check(lib().synim_interaction_matrix_repaired(geom._h, cube.data_ptr(), n, bptr, dptr, int(bbox_max[0]),
+                                                       int(bbox_max[1]), arr, repair_mask.data_ptr(), float(threshold),
+                                                       out.data_ptr(), ld, _stream_ptr(stream)))
+        return out
     _check(lib().synim_interaction_matrix(geom._h, cube.data_ptr(), n, bptr, dptr, int(bbox_max[0]), int(bbox_max[1]),
                                           arr, int(mode), out.data_ptr(), ld, _stream_ptr(stream)))
     return out

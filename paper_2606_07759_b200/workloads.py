@@ -82,6 +82,8 @@ class Workload:
     bbox: Optional[np.ndarray]       # int32 [n_modes][4] (x0,y0,x1,y1 inclusive) or None (dense)
     wfs: List[WfsInput] = field(default_factory=list)
     mode_ids: Optional[np.ndarray] = None   # index of each kept mode in the full config
+    mask: Optional[np.ndarray] = None       # float32 [ny][nx]: the modes exist only inside this SOURCE-frame mask
+                                            # (the edge-repair case); None: defined everywhere
 
     @property
     def n_modes(self) -> int:
@@ -341,3 +343,14 @@ def random_smooth_cube(n_modes: int, ny: int, nx: int, seed: int) -> np.ndarray:
             z += rng.normal() * np.cos(fx * xx + fy * yy + rng.uniform(0, 2 * math.pi))
         cube[k] = z.astype(np.float32)
     return cube
+
+
+def masked(wl: Workload, mask: np.ndarray) -> Workload:
+    """The edge-repair variant of a workload: the same modes cut by a mask given in the source
+    frame (a DM or pupil mask; values in [0, 1]), as a real M4 influence-function file or modal basis would be.
+    Supports are recomputed (a masked influence function can only shrink)."""
+    mask = np.ascontiguousarray(mask, dtype=np.float32)
+    assert mask.shape == (wl.ny, wl.nx)
+    cube = np.ascontiguousarray(wl.cube * mask[None], dtype=np.float32)
+    bbox = None if wl.bbox is None else tight_bboxes(cube)
+    return Workload(wl.name + ", masked", wl.cfg, wl.ny, wl.nx, cube, bbox, wl.wfs, wl.mode_ids, mask)

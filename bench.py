@@ -186,6 +186,12 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--parity-modes", type=int, default=256)
+    ap.add_argument("--repair", action="store_true",
+                    help="time synim_interaction_matrix_repaired (edge repair, PAPER.md:69-76) on the config's modes cut by "
+                         "a source-frame pupil mask instead of the plain hot path")
+    ap.add_argument("--dictionary", type=int, default=0, metavar="MODES_PER_LAYER",
+                    help="also run the 12-layer dictionary of PAPER.md:132 (workloads.make_dictionary, this many modes per "
+                         "layer) through synim_dictionary_host and report it under config.dictionary")
     ap.add_argument("--slope-mode", default="nd", choices=["nd", "gtilt"],
                     help="nd = the paper's numerical-derivative engine (the metric); gtilt = the comparison estimator")
     args = ap.parse_args()
@@ -217,6 +223,13 @@ def main():
 
     # every rank: its own workload of the same shape (independent problems -> weak scaling)
     wl = workloads.make_config(args.config)
+    repair_mask = None
+    if args.repair:
+        if args.slope_mode != "nd":
+            raise SystemExit("bench.py: --repair belongs to the numerical-derivative engine")
+        # the modes cut by a round mask in the source frame, 1 % inside the grid's edge (a DM / pupil mask)
+        wl = workloads.masked(wl, workloads.make_pupil(wl.nx, 0.99 * wl.nx, 0.0) if wl.ny == wl.nx else np.ones((wl.ny, wl.nx), np.float32))
+        repair_mask = torch.from_numpy(wl.mask).cuda()
     affines = synim.affines_of(wl)
     scales = [w.slope_scale for w in wl.wfs]
     stream = torch.cuda.current_stream()
@@ -235,7 +248,8 @@ def main():
         bbox, diag = synim.compute_supports(cube)
         bmax = synim.bbox_extent(bbox)
     smode = synim.SLOPES_GTILT if args.slope_mode == "gtilt" else synim.SLOPES_ND
-    synim.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax, stream=stream, diag=diag, mode=smode)
+    synim.interaction_matrix(geom, cube, bbox, affines, scales, out=out, bbox_max=bmax, stream=stream, diag=diag, mode=smode,
+                             repair_mask=repair_mask)
     e1.record(stream)
     torch.cuda.synchronize()
     first_call = {"wall_ms": 1e3 * (time.perf_counter() - t_first0), "device_ms": e0.elapsed_time(e1),
@@ -244,7 +258,8 @@ def main():
     assert geom.num_rows == wl.n_rows
 
     def step(o=out, c=cube, b=bbox, d=diag):
-        synim.interaction_matrix(geom, c, b, affines, scales, out=o, bbox_max=bmax, stream=stream, diag=d, mode=smode)
+        synim.interaction_matrix(geom, c, b, affines, scales, out=o, bbox_max=bmax, stream=stream, diag=d, mode=smode,
+                                 repair_mask=repair_mask)
 
     launches0 = synim.launch_count()
     step()
@@ -317,7 +332,8 @@ def main():
         from oracle import oracle as O
         rng = np.random.default_rng(7759 + 100)
         sel = np.sort(rng.choice(wl.n_modes, size=min(args.parity_modes, wl.n_modes), replace=False))
-        ref = O.interaction_matrix(wl, modes=sel, mode=O.GTILT if args.slope_mode == "gtilt" else O.ND)
+        ref = O.interaction_matrix(wl, modes=sel, mode=O.GTILT if args.slope_mode == "gtilt" else O.ND,
+                                   repair_mask=wl.mask if args.repair else None)
         got = out[torch.from_numpy(sel).cuda()].cpu().numpy().T.astype(np.float64)
         amp = np.abs(wl.cube[sel]).reshape(len(sel), -1).max(axis=1)
         l2w = elw = 0.0
@@ -334,6 +350,8 @@ def main():
 
     # end to end through the HOST-buffer entry point (pinned host memory, copies inside the timing)
     e2e = None
+    if args.repair:
+        args.no_e2e = True     # the host-buffer entry points have no repaired variant
     if not args.no_e2e:
         h_cube = torch.from_numpy(wl.cube).pin_memory()
         h_bbox = None if wl.bbox is None else torch.from_numpy(wl.bbox).pin_memory()
@@ -363,6 +381,35 @@ def main():
             e2e_parity = float((np.abs(got_h - got).max(axis=0) / np.maximum(cmx, 1e-30)).max())
         e2e = (e2e_ms, h2d, d2h, host_in, e2e_parity)
 
+    # the multi-layer dictionary of PAPER.md:132-138, end to end through host buffers (optional)
+    dictionary = None
+    if args.dictionary > 0 and rank == 0:
+        layers = workloads.make_dictionary(n_layers=12, max_modes=args.dictionary)
+        dgeom = synim.create_geometry(layers[0].ny, layers[0].nx, layers[0].wfs)
+        spec = [dict(cube=torch.from_numpy(l.cube).pin_memory(), bbox=torch.from_numpy(l.bbox).pin_memory(),
+                     affines=synim.affines_of(l),
+                     out=torch.empty((l.n_modes, dgeom.num_rows), dtype=torch.float32).pin_memory()) for l in layers]
+        synim.dictionary_host(dgeom, spec, stream=stream)      # warm-up: buffers, module load
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        synim.dictionary_host(dgeom, spec, stream=stream)
+        torch.cuda.synchronize()
+        d_ms = 1e3 * (time.perf_counter() - t0)
+        n_cols = sum(l.n_columns for l in layers)
+        d2h = sum(l.n_modes for l in layers) * dgeom.num_rows * 4
+        from oracle import oracle as O2
+        l0 = layers[-1]
+        pick = np.arange(min(4, l0.n_modes))
+        refd = O2.interaction_matrix(l0, modes=pick)
+        gotd = spec[-1]["out"][: len(pick)].numpy().T.astype(np.float64)
+        dictionary = {"layers": len(layers), "grids": [l.ny for l in layers], "modes_per_layer": [l.n_modes for l in layers],
+                      "columns": n_cols, "ms": d_ms, "columns_per_s": n_cols / (d_ms * 1e-3),
+                      "host_cube_bytes": int(sum(l.cube.nbytes for l in layers)), "d2h_bytes": int(d2h),
+                      "d2h_gbs": d2h / (d_ms * 1e-3) / 1e9,
+                      "top_layer_max_abs_err_vs_oracle": float(np.abs(gotd - refd).max() / np.abs(refd).max()),
+                      "api": "synim_dictionary_host (pinned host buffers, chunks of 64 MB of matrix, two in flight)"}
+        dgeom.destroy()
+
     times = torch.tensor([float(cold.mean()), e2e[0] if e2e else 0.0, float(warm.mean()), strong_ms], dtype=torch.float64,
                          device="cuda")
     if dist is not None:
@@ -383,6 +430,10 @@ def main():
                  "cold_ms_min_med_max": [float(cold.min()), float(np.median(cold)), float(cold.max())],
                  "warm_ms_per_step": warm_ms, "warm_ms_min_med_max": [float(warm.min()), float(np.median(warm)), float(warm.max())],
                  "first_call": first_call}
+        if dictionary:
+            extra["dictionary"] = dictionary
+        if args.repair:
+            extra["edge_repair"] = "synim_interaction_matrix_repaired, threshold 0.999999, modes cut by a round source-frame mask"
         if world > 1:
             extra["strong_scaling"] = {"what": "ONE cube sharded by contiguous mode ranges (sharding.partition_modes), cold L2, "
                                                "max over ranks", "ms_per_step": strong_ms,
@@ -408,7 +459,7 @@ def main():
                            "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2], "ms_per_step": e2e_ms,
                            "host_input_bytes": e2e[3], "max_elementwise_vs_device_path": e2e[4],
                            "api": "synim_interaction_matrix_host (pinned host buffers; compact supports are packed "
-                                  "on the host and only they cross the bus)"}
+                                  "on the host and only they cross the bus; chunks of modes pipelined: pack | H2D + kernel | D2H)"}
         if world == 1 and not args.no_cpu_baseline:
             v, cores, desc = oracle_throughput(wl, 10.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}

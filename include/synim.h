@@ -176,11 +176,32 @@ synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *
  * INVALID_ARG) only the supports cross the bus: each mode's bbox plus the ring of zeros the kernel stages
  * with it is packed into a pinned buffer of [n_modes][max_h + 2][roundup4(max_w + 5)] floats (host
  * threads), copied, and the kernel reads the packed cube through per-mode origins.  With h_bbox == NULL
- * (dense modes) the whole cube is copied.  Pinned h_influence / h_out make the copies asynchronous but
- * are not required. */
+ * (dense modes) the whole cube is copied.  The modes are processed in chunks whose packing, copies and kernels
+ * overlap (see synim_dictionary_host).  Pinned h_influence / h_out make the copies asynchronous but are not required. */
 synim_status synim_interaction_matrix_host(const synim_geometry *geom, const float *h_influence, int32_t n_modes,
                                            const int32_t *h_bbox, const synim_wfs_affine *affine,
                                            synim_slope_mode mode, float *h_out, void *stream);
+
+/* One component of a multi-layer dictionary (sec. 4.2: DMs and atmospheric layers at different
+ * conjugation altitudes, each with its own meta-pupil grid, modes and per-sensor composite transforms). */
+typedef struct {
+    const float *h_influence;         /* HOST float32 [n_modes][ny][nx] */
+    int32_t n_modes, ny, nx;          /* nx % 4 == 0; the layer's own source grid (the geometry's is not used) */
+    const int32_t *h_bbox;            /* HOST int32 [n_modes][4] inside the grid, or NULL = dense modes */
+    const synim_wfs_affine *affine;   /* HOST [n_wfs]: this layer's composite transforms (cone factor, footprints ...) */
+    float *h_out;                     /* HOST float32, column-major, ld = synim_num_rows(): the layer's own matrix */
+} synim_layer;
+
+/* The whole dictionary in one call, HOST buffers in and out: every layer's cube is fetched exactly once for all
+ * sensors and streamed -- the modes of all layers are cut into chunks of about 64 MB of matrix, and
+ * while chunk k is packed on the host (compact supports only) and copied in, chunk k-1 is computed and chunk k-2's
+ * columns travel back, on two internal streams with two buffers of everything.  The sensors (geometry) are shared by
+ * all layers; only the per-layer transforms differ.  Work queued on `stream` before the call is waited for; the call
+ * returns when every matrix is in host memory.  synim_interaction_matrix_host is this call with one layer on the
+ * geometry's own grid.  Pinned host buffers make the copies asynchronous but are not required.
+ * Errors: INVALID_ARG (NULL, sizes, a bbox that leaves its grid, singular affine), ALIGNMENT, OUT_OF_MEMORY, CUDA. */
+synim_status synim_dictionary_host(const synim_geometry *geom, const synim_layer *layers, int32_t n_layers,
+                                   synim_slope_mode mode, void *stream);
 
 void synim_destroy(synim_geometry *geom); /* NULL-safe; frees the internal device buffers */
 const char *synim_last_error(void);       /* thread-local, never NULL */

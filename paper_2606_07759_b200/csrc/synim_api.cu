@@ -58,16 +58,18 @@ struct synim_geometry {
     int ny = 0, nx = 0, device = 0;
     long long rows = 0;
     std::vector<WfsHost> wfs;
-    // grow-only device workspace of synim_interaction_matrix_host / synim_bbox_extent
-    mutable std::mutex lock;
-    mutable float *ws_cube = nullptr;
-    mutable size_t ws_cube_bytes = 0;
-    mutable float *ws_out = nullptr;
-    mutable size_t ws_out_bytes = 0;
-    mutable int *ws_bbox = nullptr;      // bboxes [n][4], then origins [n][2]
-    mutable size_t ws_bbox_bytes = 0;
-    mutable float *h_stage = nullptr;    // pinned: the packed supports on their way to the device
-    mutable size_t h_stage_bytes = 0;
+    mutable std::mutex lock;   // one host-buffer call at a time per geometry (they share the pipeline's buffers)
+    // the host entry points' pipeline (synim_interaction_matrix_host / synim_dictionary_host): two chunks in flight
+    struct Pipe {
+        bool ready = false;
+        cudaStream_t s_compute = nullptr, s_copy = nullptr;
+        cudaEvent_t start = nullptr, h2d_done[2] = {nullptr, nullptr}, kern_done[2] = {nullptr, nullptr}, d2h_done[2] = {nullptr, nullptr};
+        float *d_cube[2] = {nullptr, nullptr}; size_t d_cube_bytes[2] = {0, 0};
+        float *d_out[2] = {nullptr, nullptr};  size_t d_out_bytes[2] = {0, 0};
+        int *d_meta[2] = {nullptr, nullptr};   size_t d_meta_bytes[2] = {0, 0};
+        char *h_stage[2] = {nullptr, nullptr}; size_t h_stage_bytes[2] = {0, 0};
+    };
+    mutable Pipe pipe;
 };
 
 namespace {
@@ -200,10 +202,19 @@ void synim_destroy(synim_geometry *g)
         if (w.d_gy) cudaFree(w.d_gy);
         if (w.d_subap_row) cudaFree(w.d_subap_row);
     }
-    if (g->ws_cube) cudaFree(g->ws_cube);
-    if (g->ws_out) cudaFree(g->ws_out);
-    if (g->ws_bbox) cudaFree(g->ws_bbox);
-    if (g->h_stage) cudaFreeHost(g->h_stage);
+    synim_geometry::Pipe &pp = g->pipe;
+    for (int b = 0; b < 2; ++b) {
+        if (pp.d_cube[b]) cudaFree(pp.d_cube[b]);
+        if (pp.d_out[b]) cudaFree(pp.d_out[b]);
+        if (pp.d_meta[b]) cudaFree(pp.d_meta[b]);
+        if (pp.h_stage[b]) cudaFreeHost(pp.h_stage[b]);
+        if (pp.h2d_done[b]) cudaEventDestroy(pp.h2d_done[b]);
+        if (pp.kern_done[b]) cudaEventDestroy(pp.kern_done[b]);
+        if (pp.d2h_done[b]) cudaEventDestroy(pp.d2h_done[b]);
+    }
+    if (pp.start) cudaEventDestroy(pp.start);
+    if (pp.s_compute) cudaStreamDestroy(pp.s_compute);
+    if (pp.s_copy) cudaStreamDestroy(pp.s_copy);
     delete g;
 }
 
@@ -362,7 +373,8 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
                                            const int32_t *d_origin, int32_t n_modes, const int32_t *d_bbox,
                                            const int32_t *d_diag, int32_t bbox_max_w, int32_t bbox_max_h,
                                            const synim_wfs_affine *affine, synim_slope_mode mode, float *d_out, int64_t ld,
-                                           void *stream, const float *d_mask = nullptr, double threshold = 0.0)
+                                           void *stream, const float *d_mask = nullptr, double threshold = 0.0,
+                                           int src_ny = 0, int src_nx = 0)
 {
     if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL geometry/affine or n_modes < 0");
     const bool repair = d_mask != nullptr;
@@ -389,7 +401,8 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int n_wfs = (int)g->wfs.size();
     const bool dense = (d_bbox == nullptr);
-    const int ny = g->ny, nx = g->nx;
+    // (a dictionary layer brings its own source grid; everything the geometry holds belongs to the sensors)
+    const int ny = src_ny > 0 ? src_ny : g->ny, nx = src_nx > 0 ? src_nx : g->nx;
 
     // ---- shared-memory sizing ------------------------------------------------------------------
     // The staged box: <= 3 columns of TMA alignment slack, ring, support (or a piece of it), ring.  With a
@@ -651,6 +664,170 @@ synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *
     return SYNIM_OK;
 }
 
+// The pipeline behind both host entry points.  The modes of every layer are cut into chunks; chunk k is packed on the
+// host (compact supports only) while chunk k-1 runs and chunk k-2 goes home:
+//     host: pack k | s_compute: H2D k, kernel k | s_copy: D2H k        (two buffers of everything, events between)
+// so the bus carries the matrix back (the bulk of the bytes) while the next supports are packed, copied and computed.
+#define SYNIM_PIPE(call)                                              \
+    do {                                                              \
+        cudaError_t e_ = (call);                                      \
+        if (e_ != cudaSuccess) return drain(cuda_fail(e_, #call));    \
+    } while (0)
+static synim_status host_pipeline(const synim_geometry *g, const synim_layer *layers, int32_t n_layers, synim_slope_mode mode,
+                                  void *stream)
+{
+    std::lock_guard<std::mutex> guard(g->lock);
+    synim_geometry::Pipe &pp = g->pipe;
+    if (!pp.ready) {
+        SYNIM_CUDA(cudaStreamCreateWithFlags(&pp.s_compute, cudaStreamNonBlocking));
+        SYNIM_CUDA(cudaStreamCreateWithFlags(&pp.s_copy, cudaStreamNonBlocking));
+        SYNIM_CUDA(cudaEventCreateWithFlags(&pp.start, cudaEventDisableTiming));
+        for (int b = 0; b < 2; ++b) {
+            SYNIM_CUDA(cudaEventCreateWithFlags(&pp.h2d_done[b], cudaEventDisableTiming));
+            SYNIM_CUDA(cudaEventCreateWithFlags(&pp.kern_done[b], cudaEventDisableTiming));
+            SYNIM_CUDA(cudaEventCreateWithFlags(&pp.d2h_done[b], cudaEventDisableTiming));
+        }
+        pp.ready = true;
+    }
+    // whatever the caller queued on `stream` comes first
+    SYNIM_CUDA(cudaEventRecord(pp.start, static_cast<cudaStream_t>(stream)));
+    SYNIM_CUDA(cudaStreamWaitEvent(pp.s_compute, pp.start, 0));
+
+    auto grow_pinned = [&](int b, size_t want) -> synim_status {
+        if (want <= pp.h_stage_bytes[b]) return SYNIM_OK;
+        if (pp.h_stage[b]) cudaFreeHost(pp.h_stage[b]);
+        pp.h_stage[b] = nullptr; pp.h_stage_bytes[b] = 0;
+        cudaError_t e = cudaMallocHost(reinterpret_cast<void **>(&pp.h_stage[b]), want);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMallocHost(staging)");
+        pp.h_stage_bytes[b] = want;
+        return SYNIM_OK;
+    };
+    auto drain = [&](synim_status st) {   // buffers are reused by the next call: nothing may still be in flight
+        cudaStreamSynchronize(pp.s_compute);
+        cudaStreamSynchronize(pp.s_copy);
+        return st;
+    };
+
+    size_t kChunkBytes = (size_t)64 << 20;   // of matrix (and of dense cube) per chunk
+    if (const char *env = std::getenv("SYNIM_HOST_CHUNK_BYTES")) {   // tuning / test knob
+        const long long v = std::atoll(env);
+        if (v >= 4096) kChunkBytes = (size_t)v;
+    }
+    const int nthreads = (int)std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
+    long long k = 0;                                // chunks issued so far (buffer = k & 1)
+    bool used[2] = {false, false};
+    for (int32_t li = 0; li < n_layers; ++li) {
+        const synim_layer &L = layers[li];
+        if (L.n_modes == 0) continue;
+        const int ny = L.ny, nx = L.nx;
+        const size_t col_bytes = sizeof(float) * (size_t)g->rows;
+        const bool dense = L.h_bbox == nullptr;
+        // compact supports: every mode of the layer is packed into one pny x pnx image (see the header)
+        int bw = 0, bh = 0, pnx = 0, pny = 0;
+        if (!dense) {
+            for (int m = 0; m < L.n_modes; ++m) {
+                const int32_t *b = L.h_bbox + 4 * (size_t)m;
+                if (b[2] < b[0] || b[3] < b[1]) continue;
+                if (b[0] < 0 || b[1] < 0 || b[2] >= nx || b[3] >= ny)
+                    return drain(fail(SYNIM_ERR_INVALID_ARG, "host entry point: layer %d: bbox of mode %d leaves the grid", (int)li, m));
+                bw = std::max(bw, b[2] - b[0] + 1);
+                bh = std::max(bh, b[3] - b[1] + 1);
+            }
+            pnx = std::max(8, (bw + 5 + 3) & ~3); pny = std::max(4, bh + 2);
+        }
+        const size_t img = dense ? (size_t)ny * nx : (size_t)pnx * pny;
+        size_t per_mode = std::max(col_bytes, dense ? sizeof(float) * img : (size_t)1);
+        const int chunk_modes = (int)std::max<size_t>(1, std::min<size_t>((size_t)L.n_modes, kChunkBytes / std::max<size_t>(per_mode, 1)));
+        for (int m0 = 0; m0 < L.n_modes; m0 += chunk_modes, ++k) {
+            const int b = (int)(k & 1), nm = std::min(chunk_modes, L.n_modes - m0);
+            const size_t cube_bytes = sizeof(float) * img * nm, meta_bytes = dense ? 0 : sizeof(int) * 6 * (size_t)nm;
+            const size_t out_bytes = col_bytes * nm;
+            synim_status st;
+            if ((st = grow(pp.d_out[b], pp.d_out_bytes[b], std::max<size_t>(out_bytes, 16))) != SYNIM_OK) return drain(st);
+            if ((st = grow(pp.d_cube[b], pp.d_cube_bytes[b], cube_bytes)) != SYNIM_OK) return drain(st);
+            const float *src_chunk = L.h_influence + (size_t)m0 * ny * nx;
+            if (dense) {
+                // the staging buffer of two chunks ago is free once its copy has left the host
+                if (used[b]) SYNIM_PIPE(cudaEventSynchronize(pp.h2d_done[b]));
+                SYNIM_PIPE(cudaMemcpyAsync(pp.d_cube[b], src_chunk, cube_bytes, cudaMemcpyHostToDevice, pp.s_compute));
+                SYNIM_PIPE(cudaEventRecord(pp.h2d_done[b], pp.s_compute));
+            } else {
+                if ((st = grow(pp.d_meta[b], pp.d_meta_bytes[b], meta_bytes)) != SYNIM_OK) return drain(st);
+                if (used[b]) SYNIM_PIPE(cudaEventSynchronize(pp.h2d_done[b]));
+                if ((st = grow_pinned(b, cube_bytes + meta_bytes)) != SYNIM_OK) return drain(st);
+                float *stage = reinterpret_cast<float *>(pp.h_stage[b]);
+                int *meta = reinterpret_cast<int *>(pp.h_stage[b] + cube_bytes);
+                std::memcpy(meta, L.h_bbox + 4 * (size_t)m0, sizeof(int) * 4 * (size_t)nm);
+                int *origin = meta + 4 * (size_t)nm;
+                auto pack = [&](int q0, int q1) {
+                    for (int q = q0; q < q1; ++q) {
+                        const int32_t *bb = L.h_bbox + 4 * (size_t)(m0 + q);
+                        float *dst = stage + img * q;
+                        std::memset(dst, 0, sizeof(float) * img);
+                        origin[2 * q] = 0; origin[2 * q + 1] = 0;
+                        if (bb[2] < bb[0] || bb[3] < bb[1]) continue;
+                        const int ox = (bb[0] - 1) & ~3, oy = bb[1] - 1;
+                        origin[2 * q] = ox; origin[2 * q + 1] = oy;
+                        const float *src = src_chunk + (size_t)q * ny * nx;
+                        const size_t row_bytes = sizeof(float) * (size_t)(bb[2] - bb[0] + 1);
+                        for (int y = bb[1]; y <= bb[3]; ++y)
+                            std::memcpy(dst + (size_t)(y - oy) * pnx + (bb[0] - ox), src + (size_t)y * nx + bb[0], row_bytes);
+                    }
+                };
+                int done = 0;   // modes [0, done) of the chunk are packed (or handed to a thread)
+                if (nthreads > 1 && nm >= 64) {
+                    std::vector<std::thread> pool;
+                    try {   // no exception crosses the C ABI: what the threads could not be started for is packed here
+                        pool.reserve(nthreads);
+                        for (int t = 0; t < nthreads; ++t) {
+                            const int q1 = (int)((long long)nm * (t + 1) / nthreads);
+                            pool.emplace_back(pack, done, q1);
+                            done = q1;
+                        }
+                    } catch (...) {
+                    }
+                    for (auto &th : pool) th.join();
+                }
+                pack(done, nm);
+                SYNIM_PIPE(cudaMemcpyAsync(pp.d_cube[b], stage, cube_bytes, cudaMemcpyHostToDevice, pp.s_compute));
+                SYNIM_PIPE(cudaMemcpyAsync(pp.d_meta[b], meta, meta_bytes, cudaMemcpyHostToDevice, pp.s_compute));
+                SYNIM_PIPE(cudaEventRecord(pp.h2d_done[b], pp.s_compute));
+            }
+            // the output buffer of two chunks ago must have gone home before the kernel overwrites it
+            if (used[b]) SYNIM_PIPE(cudaStreamWaitEvent(pp.s_compute, pp.d2h_done[b], 0));
+            if (dense)
+                st = run_interaction_matrix(g, pp.d_cube[b], ny, nx, nullptr, nm, nullptr, nullptr, 0, 0, L.affine, mode, pp.d_out[b],
+                                            g->rows, pp.s_compute, nullptr, 0.0, ny, nx);
+            else
+                st = run_interaction_matrix(g, pp.d_cube[b], pny, pnx, pp.d_meta[b] + 4 * (size_t)nm, nm, pp.d_meta[b], nullptr, bw, bh,
+                                            L.affine, mode, pp.d_out[b], g->rows, pp.s_compute, nullptr, 0.0, ny, nx);
+            if (st != SYNIM_OK) return drain(st);
+            SYNIM_PIPE(cudaEventRecord(pp.kern_done[b], pp.s_compute));
+            SYNIM_PIPE(cudaStreamWaitEvent(pp.s_copy, pp.kern_done[b], 0));
+            SYNIM_PIPE(cudaMemcpyAsync(L.h_out + (size_t)m0 * (size_t)g->rows, pp.d_out[b], out_bytes, cudaMemcpyDeviceToHost, pp.s_copy));
+            SYNIM_PIPE(cudaEventRecord(pp.d2h_done[b], pp.s_copy));
+            used[b] = true;
+        }
+    }
+    cudaError_t e1 = cudaStreamSynchronize(pp.s_compute), e2 = cudaStreamSynchronize(pp.s_copy);
+    if (e1 != cudaSuccess) return cuda_fail(e1, "cudaStreamSynchronize(compute)");
+    if (e2 != cudaSuccess) return cuda_fail(e2, "cudaStreamSynchronize(copy)");
+    return SYNIM_OK;
+}
+
+static synim_status check_layers(const synim_geometry *g, const synim_layer *layers, int32_t n_layers, const char *who)
+{
+    for (int32_t li = 0; li < n_layers; ++li) {
+        const synim_layer &L = layers[li];
+        if (L.n_modes < 0 || L.ny <= 0 || L.nx <= 0) return fail(SYNIM_ERR_INVALID_ARG, "%s: layer %d: bad sizes", who, (int)li);
+        if (L.nx % 4 != 0) return fail(SYNIM_ERR_ALIGNMENT, "%s: layer %d: nx = %d is not a multiple of 4", who, (int)li, L.nx);
+        if (L.n_modes > 0 && (!L.h_influence || !L.h_out || !L.affine))
+            return fail(SYNIM_ERR_INVALID_ARG, "%s: layer %d: NULL host buffer or affine", who, (int)li);
+    }
+    (void)g;
+    return SYNIM_OK;
+}
+
 synim_status synim_interaction_matrix_host(const synim_geometry *g, const float *h_influence, int32_t n_modes,
                                            const int32_t *h_bbox, const synim_wfs_affine *affine, synim_slope_mode mode,
                                            float *h_out, void *stream)
@@ -658,92 +835,20 @@ synim_status synim_interaction_matrix_host(const synim_geometry *g, const float 
     if (!g || !affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_host: bad arguments");
     if (n_modes == 0) return SYNIM_OK;
     if (!h_influence || !h_out) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_host: NULL host buffer");
-    cudaStream_t s = static_cast<cudaStream_t>(stream);
-    std::lock_guard<std::mutex> guard(g->lock);
-    const int ny = g->ny, nx = g->nx;
-    const size_t out_bytes = sizeof(float) * (size_t)n_modes * (size_t)g->rows;
-    synim_status st;
-    if ((st = grow(g->ws_out, g->ws_out_bytes, std::max<size_t>(out_bytes, 16))) != SYNIM_OK) return st;
+    synim_layer L;
+    L.h_influence = h_influence; L.n_modes = n_modes; L.ny = g->ny; L.nx = g->nx; L.h_bbox = h_bbox; L.affine = affine; L.h_out = h_out;
+    return host_pipeline(g, &L, 1, mode, stream);
+}
 
-    if (!h_bbox) {   // dense modes: the whole cube crosses the bus
-        const size_t cube_bytes = sizeof(float) * (size_t)n_modes * ny * nx;
-        if ((st = grow(g->ws_cube, g->ws_cube_bytes, cube_bytes)) != SYNIM_OK) return st;
-        SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, h_influence, cube_bytes, cudaMemcpyHostToDevice, s));
-        st = run_interaction_matrix(g, g->ws_cube, ny, nx, nullptr, n_modes, nullptr, nullptr, 0, 0, affine, mode, g->ws_out,
-                                    g->rows, s);
-    } else {
-        // Compact supports: only each mode's bbox (plus the ring of zeros the kernel stages with it) crosses
-        // the bus -- 29 MB instead of 4.67 GB at config 3.  Mode m is packed into a pny x pnx image whose
-        // pixel (0, 0) is source pixel (ox, oy) = ((x0-1) & ~3, y0-1): exactly the origin of the box the
-        // kernel's TMA load asks for, 16-byte aligned like it.
-        int bw = 0, bh = 0;
-        for (int m = 0; m < n_modes; ++m) {
-            const int32_t *b = h_bbox + 4 * (size_t)m;
-            if (b[2] < b[0] || b[3] < b[1]) continue;
-            if (b[0] < 0 || b[1] < 0 || b[2] >= nx || b[3] >= ny)
-                return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_host: bbox of mode %d leaves the grid", m);
-            bw = std::max(bw, b[2] - b[0] + 1);
-            bh = std::max(bh, b[3] - b[1] + 1);
-        }
-        const int pnx = std::max(8, (bw + 5 + 3) & ~3), pny = std::max(4, bh + 2);
-        const size_t img = (size_t)pnx * pny, cube_bytes = sizeof(float) * img * n_modes;
-        const size_t meta_bytes = sizeof(int) * 6 * (size_t)n_modes;   // bboxes [n][4], origins [n][2]
-        if ((st = grow(g->ws_cube, g->ws_cube_bytes, cube_bytes)) != SYNIM_OK) return st;
-        if ((st = grow(g->ws_bbox, g->ws_bbox_bytes, meta_bytes)) != SYNIM_OK) return st;
-        if (g->h_stage_bytes < cube_bytes + meta_bytes) {
-            if (g->h_stage) cudaFreeHost(g->h_stage);
-            g->h_stage = nullptr; g->h_stage_bytes = 0;
-            cudaError_t e = cudaMallocHost(reinterpret_cast<void **>(&g->h_stage), cube_bytes + meta_bytes);
-            if (e != cudaSuccess) return cuda_fail(e, "cudaMallocHost(staging)");
-            g->h_stage_bytes = cube_bytes + meta_bytes;
-        }
-        float *stage = g->h_stage;
-        int *meta = reinterpret_cast<int *>(reinterpret_cast<char *>(g->h_stage) + cube_bytes);
-        std::memcpy(meta, h_bbox, sizeof(int) * 4 * (size_t)n_modes);
-        int *origin = meta + 4 * (size_t)n_modes;
-        auto pack = [&](int m0, int m1) {
-            for (int m = m0; m < m1; ++m) {
-                const int32_t *b = h_bbox + 4 * (size_t)m;
-                float *dst = stage + img * m;
-                std::memset(dst, 0, sizeof(float) * img);
-                origin[2 * m] = 0; origin[2 * m + 1] = 0;
-                if (b[2] < b[0] || b[3] < b[1]) continue;
-                const int ox = (b[0] - 1) & ~3, oy = b[1] - 1;
-                origin[2 * m] = ox; origin[2 * m + 1] = oy;
-                const float *src = h_influence + (size_t)m * ny * nx;
-                const size_t row_bytes = sizeof(float) * (size_t)(b[2] - b[0] + 1);
-                for (int y = b[1]; y <= b[3]; ++y)
-                    std::memcpy(dst + (size_t)(y - oy) * pnx + (b[0] - ox), src + (size_t)y * nx + b[0], row_bytes);
-            }
-        };
-        const int nthreads = (int)std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
-        int done = 0;   // modes [0, done) are packed (or handed to a thread)
-        if (nthreads > 1 && n_modes >= 64) {
-            std::vector<std::thread> pool;
-            try {   // no exception crosses the C ABI: what the threads could not be started for is packed here
-                pool.reserve(nthreads);
-                for (int t = 0; t < nthreads; ++t) {
-                    const int m1 = (int)((long long)n_modes * (t + 1) / nthreads);
-                    pool.emplace_back(pack, done, m1);
-                    done = m1;
-                }
-            } catch (...) {
-            }
-            for (auto &th : pool) th.join();
-        }
-        pack(done, n_modes);
-        SYNIM_CUDA(cudaMemcpyAsync(g->ws_cube, stage, cube_bytes, cudaMemcpyHostToDevice, s));
-        SYNIM_CUDA(cudaMemcpyAsync(g->ws_bbox, meta, meta_bytes, cudaMemcpyHostToDevice, s));
-        st = run_interaction_matrix(g, g->ws_cube, pny, pnx, g->ws_bbox + 4 * (size_t)n_modes, n_modes, g->ws_bbox, nullptr, bw, bh,
-                                    affine, mode, g->ws_out, g->rows, s);
-    }
-    if (st != SYNIM_OK) {
-        cudaStreamSynchronize(s);   // the staging buffers may still be in flight: they are reused by the next call
-        return st;
-    }
-    SYNIM_CUDA(cudaMemcpyAsync(h_out, g->ws_out, out_bytes, cudaMemcpyDeviceToHost, s));
-    SYNIM_CUDA(cudaStreamSynchronize(s));
-    return SYNIM_OK;
+synim_status synim_dictionary_host(const synim_geometry *g, const synim_layer *layers, int32_t n_layers, synim_slope_mode mode,
+                                   void *stream)
+{
+    if (!g || n_layers < 0 || (n_layers > 0 && !layers)) return fail(SYNIM_ERR_INVALID_ARG, "synim_dictionary_host: bad arguments");
+    if (mode != SYNIM_SLOPES_ND && mode != SYNIM_SLOPES_GTILT) return fail(SYNIM_ERR_INVALID_ARG, "synim_dictionary_host: unknown slope mode %d", (int)mode);
+    synim_status st = check_layers(g, layers, n_layers, "synim_dictionary_host");
+    if (st != SYNIM_OK) return st;
+    if (n_layers == 0) return SYNIM_OK;
+    return host_pipeline(g, layers, n_layers, mode, stream);
 }
 
 }  // extern "C"

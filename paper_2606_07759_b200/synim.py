@@ -23,7 +23,7 @@ SLOPES_ND, SLOPES_GTILT = 0, 1
 EXPORTS = ("synim_compose_affine", "synim_create_geometry", "synim_num_rows", "synim_num_valid",
            "synim_row_offset", "synim_interaction_matrix", "synim_interaction_matrix_repaired", "synim_compute_bboxes",
            "synim_bbox_extent",
-           "synim_interaction_matrix_host", "synim_destroy", "synim_last_error", "synim_version",
+           "synim_interaction_matrix_host", "synim_dictionary_host", "synim_destroy", "synim_last_error", "synim_version",
            "synim_launch_count")
 
 PHYSICAL_FIELDS = ("shift_x", "shift_y", "rot_deg", "mag_x", "mag_y",
@@ -43,6 +43,12 @@ class WfsAffine(ctypes.Structure):
 
 class WfsPhysical(ctypes.Structure):
     _fields_ = [(k, ctypes.c_double) for k in PHYSICAL_FIELDS]
+
+
+class Layer(ctypes.Structure):
+    _fields_ = [("h_influence", ctypes.c_void_p), ("n_modes", ctypes.c_int32), ("ny", ctypes.c_int32),
+                ("nx", ctypes.c_int32), ("h_bbox", ctypes.c_void_p), ("affine", ctypes.POINTER(WfsAffine)),
+                ("h_out", ctypes.c_void_p)]
 
 
 class SynimError(RuntimeError):
@@ -85,6 +91,8 @@ def lib() -> ctypes.CDLL:
         L.synim_bbox_extent.argtypes = [vp, i32, ctypes.POINTER(i32), ctypes.POINTER(i32), vp]
         L.synim_interaction_matrix_host.restype = ctypes.c_int
         L.synim_interaction_matrix_host.argtypes = [vp, vp, i32, vp, ctypes.POINTER(WfsAffine), ctypes.c_int, vp, vp]
+        L.synim_dictionary_host.restype = ctypes.c_int
+        L.synim_dictionary_host.argtypes = [vp, ctypes.POINTER(Layer), i32, ctypes.c_int, vp]
         L.synim_destroy.restype = None
         L.synim_destroy.argtypes = [vp]
         L.synim_last_error.restype = ctypes.c_char_p
@@ -317,6 +325,49 @@ def interaction_matrix_host(geom: Geometry, cube_host, bbox_host, affines: Seque
                                                None if bbox_host is None else ptr(bbox_host),
                                                arr, int(mode), ptr(out_host), _stream_ptr(stream)))
     return out_host
+
+
+def dictionary_host(geom: Geometry, layers: Sequence[dict], mode: int = SLOPES_ND, stream=None):
+    """synim_dictionary_host: ``layers`` is a list of dicts with ``cube`` (host float32 [n][ny][nx], torch CPU tensor or
+    numpy), ``bbox`` (host int32 [n][4] or None), ``affines`` ([n_wfs][6]), optional ``scales`` and ``out`` (host float32
+    [n][rows]; allocated pinned if missing).  Returns the list of output buffers."""
+    import torch
+
+    def ptr(x):
+        return x.data_ptr() if isinstance(x, torch.Tensor) else x.ctypes.data
+
+    def ok(x, dt_t, dt_n):
+        if isinstance(x, torch.Tensor):
+            return (not x.is_cuda) and x.dtype == dt_t and x.is_contiguous()
+        return isinstance(x, np.ndarray) and x.dtype == dt_n and x.flags["C_CONTIGUOUS"]
+
+    rows = geom.num_rows
+    arr = (Layer * len(layers))()
+    keep, outs = [], []
+    for k, lay in enumerate(layers):
+        cube, bbox = lay["cube"], lay.get("bbox")
+        if not ok(cube, torch.float32, np.float32) or len(cube.shape) != 3:
+            raise ValueError(f"layer {k}: cube must be a C-contiguous host float32 array [n][ny][nx]")
+        n, ny, nx = (int(v) for v in cube.shape)
+        if bbox is not None and (not ok(bbox, torch.int32, np.int32) or tuple(bbox.shape) != (n, 4)):
+            raise ValueError(f"layer {k}: bbox must be a C-contiguous host int32 array [n][4]")
+        if len(lay["affines"]) != geom.n_wfs:
+            raise ValueError(f"layer {k}: one affine per sensor")
+        out = lay.get("out")
+        if out is None:
+            out = torch.empty((n, rows), dtype=torch.float32).pin_memory()
+        if not ok(out, torch.float32, np.float32) or tuple(out.shape) != (n, rows):
+            raise ValueError(f"layer {k}: out must be a C-contiguous host float32 array [{n}][{rows}]")
+        aff = _affine_array(lay["affines"], lay.get("scales"))
+        keep.append((cube, bbox, out, aff))
+        arr[k].h_influence, arr[k].n_modes, arr[k].ny, arr[k].nx = ptr(cube), n, ny, nx
+        arr[k].h_bbox = None if bbox is None else ptr(bbox)
+        arr[k].affine = ctypes.cast(aff, ctypes.POINTER(WfsAffine))
+        arr[k].h_out = ptr(out)
+        outs.append(out)
+    _check(lib().synim_dictionary_host(geom._h, arr, len(layers), int(mode), _stream_ptr(stream)))
+    del keep
+    return outs
 
 
 def affines_of(workload) -> list:

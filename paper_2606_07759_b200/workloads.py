@@ -354,3 +354,37 @@ def masked(wl: Workload, mask: np.ndarray) -> Workload:
     cube = np.ascontiguousarray(wl.cube * mask[None], dtype=np.float32)
     bbox = None if wl.bbox is None else tight_bboxes(cube)
     return Workload(wl.name + ", masked", wl.cfg, wl.ny, wl.nx, cube, bbox, wl.wfs, wl.mode_ids, mask)
+
+
+def make_dictionary(n_layers: int = 12, acts_across: int = 66, max_modes: Optional[int] = None,
+                    top_km: float = 22.0, grid_lo: int = 480, grid_hi: int = 692) -> List[Workload]:
+    """A multi-layer dictionary of the shape of PAPER.md:132 (MORFEO: 3 DMs + 9 layers = 12 altitude components
+    between 0 and 22 km, six LGS WFS of 68x68 subapertures, meta-pupil grids of 480^2 ... 690^2 pixels): one
+    Workload per component, all looking through the SAME six sensors (the config-3 sensors, 45 arcsec off axis on a
+    hexagonal ring, 90 km range), each with its own grid, cone factor and footprints (the physical records carry
+    dm_height_m).  Zonal Gaussian influence functions on a centred grid of ``acts_across`` actuators across the
+    meta-pupil; ``max_modes`` keeps a seeded subset per layer.  Stand-in for the MORFEO modal bases, which are not
+    available here."""
+    npix, nsub = 7, 68
+    m = nsub * npix
+    pup = make_pupil(m, 476.0, 0.28)
+    val = valid_subaps(pup, nsub, npix)
+    base = _cfg3_physical(7759 + 3)
+    pitch_m = 38.5 / 476.0
+    out = []
+    for li in range(n_layers):
+        h_km = top_km * li / max(1, n_layers - 1)
+        n = (int(round(grid_lo + (grid_hi - grid_lo) * h_km / top_km)) + 3) & ~3
+        d_meta = 476.0 + (n - 480.0)
+        pitch = d_meta / acts_across
+        acts = actuator_grid(acts_across + 1, pitch, d_meta / 2.0 + pitch / 2.0)
+        keep = _subset(len(acts), max_modes, 7759 + 100 + li)
+        cube, bbox = gaussian_cube(n, n, acts[keep], pitch)
+        wfs = []
+        for k, p in enumerate(base):
+            q = dict(p)
+            q.update(dm_height_m=1000.0 * h_km, gs_range_m=90000.0, gs_theta_arcsec=45.0, gs_azimuth_deg=60.0 * k,
+                     src_pixel_pitch_m=pitch_m)
+            wfs.append(WfsInput(nsub, npix, pup, val, q))
+        out.append(Workload(f"dictionary layer {li} ({h_km:.1f} km, {n}x{n})", 0, n, n, cube, bbox, wfs, keep))
+    return out

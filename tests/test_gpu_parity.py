@@ -546,3 +546,44 @@ def test_host_entry_point_packs_supports_edges_empty_modes_and_dense(S):
     out = S.interaction_matrix_host(geom, torch.from_numpy(wl.cube).pin_memory(), None, S.affines_of(wl))
     assert_parity(out.numpy().T.copy(), O.interaction_matrix(wl), wl)
     geom.destroy()
+
+
+def test_host_entry_point_in_chunks(S, monkeypatch):
+    """The host entry point's pipeline with chunks of a few modes (SYNIM_HOST_CHUNK_BYTES): buffers alternate, the
+    copies of one chunk overlap the kernel of the next, and the matrix is the same as in one piece."""
+    import torch
+    wl = W.make_config(1)
+    ref = O.interaction_matrix(wl)
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    for chunk in ("8000", "100000", None):
+        if chunk is None:
+            monkeypatch.delenv("SYNIM_HOST_CHUNK_BYTES", raising=False)
+        else:
+            monkeypatch.setenv("SYNIM_HOST_CHUNK_BYTES", chunk)
+        out = S.interaction_matrix_host(geom, torch.from_numpy(wl.cube).pin_memory(), wl.bbox, S.affines_of(wl))
+        assert_parity(out.numpy().T.copy(), ref, wl)
+        out = S.interaction_matrix_host(geom, wl.cube, None, S.affines_of(wl), mode=S.SLOPES_GTILT)     # dense, pageable
+        assert_parity(out.numpy().T.copy(), O.interaction_matrix(wl, mode=O.GTILT), wl)
+    geom.destroy()
+
+
+def test_dictionary_host_streams_layers_with_their_own_grids(S, monkeypatch):
+    """synim_dictionary_host: components at different altitudes, each with its own meta-pupil
+    grid, cone factor and footprints, through one set of sensors; a dense and an empty layer among them; every
+    layer's matrix against the oracle."""
+    layers = W.make_dictionary(n_layers=4, acts_across=40, max_modes=20)
+    dense = W.make_config(5, max_modes=2)
+    dense.wfs = layers[0].wfs                      # same sensors, the ground layer's transforms
+    layers.insert(2, dense)
+    geom = S.create_geometry(layers[0].ny, layers[0].nx, layers[0].wfs)
+    spec = [dict(cube=l.cube, bbox=l.bbox, affines=S.affines_of(l), scales=[1.0 + 0.1 * k] * len(l.wfs)) for k, l in enumerate(layers)]
+    spec.insert(1, dict(cube=np.zeros((0, 480, 480), np.float32), bbox=np.zeros((0, 4), np.int32), affines=S.affines_of(layers[0])))
+    monkeypatch.setenv("SYNIM_HOST_CHUNK_BYTES", str(6 * 40272 * 4))       # six modes per chunk
+    outs = S.dictionary_host(geom, spec)
+    outs.pop(1)
+    for k, (l, o) in enumerate(zip(layers, outs)):
+        for w in l.wfs:
+            w.slope_scale = 1.0 + 0.1 * k
+        assert_parity(o.numpy().T.copy(), O.interaction_matrix(l), l)
+    assert len({l.ny for l in layers}) >= 3 and layers[-1].wfs[0].phys["dm_height_m"] == 22000.0
+    geom.destroy()

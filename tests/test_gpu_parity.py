@@ -587,3 +587,32 @@ def test_dictionary_host_streams_layers_with_their_own_grids(S, monkeypatch):
         assert_parity(o.numpy().T.copy(), O.interaction_matrix(l), l)
     assert len({l.ny for l in layers}) >= 3 and layers[-1].wfs[0].phys["dm_height_m"] == 22000.0
     geom.destroy()
+
+
+def test_mode_ranges_through_the_library_concatenate_to_the_unsharded_matrix(S):
+    """the mode axis shards with no exchange.  The ranges of sharding.partition_modes go through
+    synim_interaction_matrix one by one (as the ranks of a job would, each on its slice of the cube and its block of
+    the column-major matrix); the concatenation equals the unsharded matrix bit for bit, zonal and dense."""
+    import torch
+    from paper_2606_07759_b200 import sharding
+    for cfg, n, dense in ((3, 61, False), (1, 23, True)):
+        wl = W.make_config(cfg, max_modes=n)
+        geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+        cube = torch.from_numpy(wl.cube).cuda()
+        bbox = diag = None
+        bmax = (0, 0)
+        if not dense:
+            bbox, diag = S.compute_supports(cube)
+            bmax = S.bbox_extent(bbox)
+        aff = S.affines_of(wl)
+        whole = S.interaction_matrix(geom, cube, bbox, aff, bbox_max=bmax, diag=diag).clone()
+        for world in (2, 3, 5):
+            out = torch.full_like(whole, float("nan"))
+            for b, e in sharding.partition_modes(wl.n_modes, world):
+                if e > b:
+                    S.interaction_matrix(geom, cube[b:e], None if bbox is None else bbox[b:e], aff, out=out[b:e],
+                                         bbox_max=bmax, diag=None if diag is None else diag[b:e])
+            torch.cuda.synchronize()
+            assert torch.equal(out, whole)
+        geom.destroy()
+    assert_parity(whole.cpu().numpy().T.copy(), O.interaction_matrix(wl), wl)

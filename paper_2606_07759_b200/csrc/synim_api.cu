@@ -358,10 +358,66 @@ static bool plan_tiles(const synim::WfsDev &d, size_t budget_floats, int reach, 
         if (ns == 1 && nr == 1) return false;
         if (nr > 1 && (nr * d.n_pix >= ns * strip_px || ns == 1)) --nr; else --ns;
     }
-    const int ty = (d.n_subap + nr - 1) / nr, tx = (n_strips + ns - 1) / ns;
-    nr = (d.n_subap + ty - 1) / ty;
-    ns = (n_strips + tx - 1) / tx;
-    box(ns, nr, &pitch, &h);
+    auto even_out = [&](int *pns, int *pnr) {
+        const int ty = (d.n_subap + *pnr - 1) / *pnr, tx = (n_strips + *pns - 1) / *pns;
+        *pnr = (d.n_subap + ty - 1) / ty;
+        *pns = (n_strips + tx - 1) / tx;
+    };
+    // Shared-memory bank conflicts of the gather.  The 32 lanes of a warp sample 32 neighbouring WFS pixels of one row;
+    // under a rotated sensor their four taps land on ~28 different box rows, and how those fall onto the 32 banks
+    // depends on the box pitch modulo 32 alone: simulated for config 5, 1.1 to 4.0 wavefronts per LDS request on the
+    // 60-degree sensors (ncu on the first version, fixed pitches: 1.9 on average).  So the pitch is padded by the
+    // multiple of 4 floats (TMA rows are 16-byte multiples) with the fewest wavefronts; if even the best one that fits
+    // stays above 1.6, a shorter tile (more room for padding) is tried.
+    auto wavefronts = [&](int pit) {
+        double tot = 0.0;
+        int cnt = 0;
+        for (int s = 0; s < 24; ++s) {
+            const double j0 = (double)((s * 37) % std::max(1, d.M - 31)), i = (double)((s * 53 + 11) % d.M);
+            long long c0[32], r0[32];
+            for (int l = 0; l < 32; ++l) {
+                const double j = j0 + l;
+                c0[l] = (long long)std::floor(d.fwd[0] * j + d.fwd[1] * i + d.fwd[2]);
+                r0[l] = (long long)std::floor(d.fwd[3] * j + d.fwd[4] * i + d.fwd[5]);
+            }
+            for (int tap = 0; tap < 4; ++tap) {
+                long long word[32];
+                int per_bank[32] = {0}, worst = 0;
+                for (int l = 0; l < 32; ++l) {
+                    word[l] = (r0[l] + (tap >> 1)) * pit + c0[l] + (tap & 1);
+                    bool seen = false;
+                    for (int q = 0; q < l && !seen; ++q) seen = word[q] == word[l];
+                    if (!seen) worst = std::max(worst, ++per_bank[(int)(((word[l] % 32) + 32) % 32)]);
+                }
+                tot += worst; ++cnt;
+            }
+        }
+        return tot / cnt;
+    };
+    auto best_pad = [&](int ns_, int nr_, int *ppitch, int *ph) {   // -> wavefronts per request; 1e9 if nothing fits
+        int p0 = 0, h0 = 0;
+        box(ns_, nr_, &p0, &h0);
+        double best = 1.0e9;
+        for (int pad = 0; pad < 32; pad += 4) {
+            const int pit = p0 + pad;
+            if (pit > 256 || h0 > 256 || (size_t)pit * h0 + 3 * (size_t)ns_ * d.spb * nr_ > budget_floats) break;
+            const double w = wavefronts(pit);
+            if (w < best - 1.0e-9) { best = w; *ppitch = pit; *ph = h0; }
+        }
+        return best;
+    };
+    even_out(&ns, &nr);
+    double got = best_pad(ns, nr, &pitch, &h);
+    for (int shorter = nr - 1; got > 1.6 && shorter >= std::max(4, nr - 3); --shorter) {
+        int ns2 = ns, nr2 = shorter, p2 = 0, h2 = 0;
+        even_out(&ns2, &nr2);
+        const double w2 = best_pad(ns2, nr2, &p2, &h2);
+        if (w2 < got - 0.2) { got = w2; ns = ns2; nr = nr2; pitch = p2; h = h2; }
+    }
+    if (got > 1.0e8) box(ns, nr, &pitch, &h);   // (cannot happen: the unpadded box of this tile fitted above)
+    if (std::getenv("SYNIM_DEBUG_TILES"))
+        std::fprintf(stderr, "synim: tile %d strips x %d rows, box %d x %d floats, %.2f shared-memory wavefronts per request\n", ns, nr,
+                     pitch, h, got);
     out->ns = ns; out->nr = nr; out->pitch = pitch; out->h = h;
     return true;
 }

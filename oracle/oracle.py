@@ -192,3 +192,33 @@ def interaction_matrix(wl, mode: int = ND, modes: Optional[Sequence[int]] = None
             blocks.append(slopes_wfs(wl.cube, w.pupil, w.n_subap, w.n_pix, w.valid, a, w.slope_scale,
                                      mode, modes, n_threads).T)
     return np.concatenate(blocks, axis=0)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Tomographic projection matrix (sec. 2.5; readings R24-R26 of DESIGN.md)
+# ------------------------------------------------------------------------------------------------------------------
+def projection_operand(cube: np.ndarray, maps: Sequence[Sequence[float]], pupil: np.ndarray,
+                       weights: Optional[Sequence[float]] = None) -> np.ndarray:
+    """P of PAPER.md:90: the influence functions of one component "mapped over the optimized directions".
+    Row (d, p) = direction d, pixel p of the mp x mp pupil grid (row-major); column m = mode m; entry
+    sqrt(w_d) * pupil[p] * phi_m(A_d x_p), phi_m resampled through the direction's composite map with the same single
+    bilinear interpolation as everywhere else (steps 1-2 of the interaction matrix, without the halo).
+    float64 [n_dir * mp * mp][n_modes]."""
+    cube = np.ascontiguousarray(cube, dtype=np.float32)
+    pupil = np.ascontiguousarray(pupil, dtype=np.float64)
+    mp = pupil.shape[0]
+    assert pupil.shape == (mp, mp)
+    n_dir = len(maps)
+    w = np.ones(n_dir) if weights is None else np.asarray(weights, dtype=np.float64)
+    out = np.empty((n_dir, mp * mp, cube.shape[0]), dtype=np.float64)
+    for d in range(n_dir):
+        for m in range(cube.shape[0]):
+            out[d, :, m] = float(np.sqrt(w[d])) * (pupil * resample(cube[m], mp, maps[d])).ravel()
+    return out.reshape(n_dir * mp * mp, cube.shape[0])
+
+
+def projection_matrix(p_dm: np.ndarray, p_layer: np.ndarray, lam: float) -> np.ndarray:
+    """P_opt = (P_DM^T P_DM + lambda I)^-1 P_DM^T P_Layer, written out as the paper gives it:
+    float64 [n_dm_modes][n_layer_modes].  P_DM holds the columns of ALL deformable mirrors side by side."""
+    g = p_dm.T @ p_dm + float(lam) * np.eye(p_dm.shape[1])
+    return np.linalg.solve(g, p_dm.T @ p_layer)

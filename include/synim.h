@@ -55,7 +55,7 @@ typedef enum {
     SYNIM_ERR_UNSUPPORTED_DEVICE = -4, /* current device is not compute capability 10.x */
     SYNIM_ERR_OUT_OF_MEMORY = -5,
     SYNIM_ERR_CUDA = -6,               /* any other CUDA runtime / driver failure */
-    SYNIM_ERR_UNSUPPORTED = -7         /* a combination that is not built: edge repair with the G-tilt estimator */
+    SYNIM_ERR_UNSUPPORTED = -7         /* edge repair with the G-tilt estimator; cuBLAS / cuSOLVER not loadable */
 } synim_status;
 
 /* Slope estimator.  ND = finite central differences averaged over the subaperture
@@ -202,6 +202,34 @@ typedef struct {
  * Errors: INVALID_ARG (NULL, sizes, a bbox that leaves its grid, singular affine), ALIGNMENT, OUT_OF_MEMORY, CUDA. */
 synim_status synim_dictionary_host(const synim_geometry *geom, const synim_layer *layers, int32_t n_layers,
                                    synim_slope_mode mode, void *stream);
+
+/* ---- Tomographic projection matrix (sec. 2.5) ------------------------------------------------------
+ * P_opt = (P_DM^T P_DM + lambda I)^-1 P_DM^T P_Layer, "where P_DM and P_Layer map the influence functions over the
+ * optimized directions".  Readings (R24-R26): row (d, p) of an operand = optimisation direction d, pixel p of
+ * an mp x mp pupil grid; column m = mode m of the component; entry = sqrt(weight_d) * pupil[p] * phi_m(A_d x_p), phi_m
+ * resampled through the direction's composite map with the library's single bilinear interpolation (zero outside the
+ * grid).  P_DM holds the columns of ALL mirrors side by side (component 0 first).
+ * One component = one deformable mirror or one reconstructed layer: */
+typedef struct {
+    const float *d_cube;            /* DEVICE float32 [n_modes][ny][nx] */
+    int32_t n_modes, ny, nx;        /* n_modes <= 65535 */
+    const synim_wfs_affine *maps;   /* HOST [n_dir]: pupil pixel -> this component's grid, centred pixel coordinates as
+                                       for a sensor (footprint h*theta of the direction, misregistration ...); slope_scale
+                                       is ignored */
+} synim_component;
+
+/* The operands are built by a kernel of this library (HBM-bound by their store); the two contractions and the Cholesky
+ * solve are cuBLAS (SYRK, GEMM, float32) and cuSOLVER (POTRF, POTRS) calls, loaded with dlopen at the first call
+ * (SYNIM_ERR_UNSUPPORTED if they cannot be found).  Temporaries (the operands: 4*n_dir*mp*mp bytes per mode) come from
+ * the stream-ordered allocator.  SYNCHRONISES `stream` once, to report a matrix that is not positive definite.
+ *   dir_weight  HOST [n_dir] non-negative weights of the directions, or NULL = all 1
+ *   d_pupil     DEVICE float32 [mp][mp] pupil weights (0 = outside)
+ *   d_popt      DEVICE float32, column-major: element (a, l) = actuator / DM mode a (all mirrors, in order), layer mode
+ *               l, at d_popt[l*ld + a]; ld >= sum of the mirrors' modes
+ * Errors: INVALID_ARG (NULL, sizes, lambda < 0, not positive definite), UNSUPPORTED, OUT_OF_MEMORY, CUDA. */
+synim_status synim_projection_matrix(const synim_component *dms, int32_t n_dms, const synim_component *layer,
+                                     int32_t n_dir, const double *dir_weight, const float *d_pupil, int32_t mp,
+                                     double lambda, float *d_popt, int64_t ld, void *stream);
 
 void synim_destroy(synim_geometry *geom); /* NULL-safe; frees the internal device buffers */
 const char *synim_last_error(void);       /* thread-local, never NULL */

@@ -14,11 +14,11 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsynim.so")
-SOURCES = ("synim_api.cu", "synim_kernels.cu", "synim_strip.cu")
+SOURCES = ("synim_api.cu", "synim_kernels.cu", "synim_strip.cu", "synim_popt.cu")
 HEADERS = ("synim_device.h", os.path.join("..", "..", "include", "synim.h"))
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC,-O2,-Wall", "--shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC,-O2,-Wall", "--shared", "-cudart", "static", "-ldl"]
 
 
 def _nvcc() -> str:

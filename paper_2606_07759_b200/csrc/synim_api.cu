@@ -36,6 +36,22 @@ synim_status cuda_fail(cudaError_t e, const char *what)
     return fail(SYNIM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+}  // namespace
+
+namespace synim {
+// the other translation units' way to set the calling thread's error text (synim_last_error)
+synim_status report(synim_status s, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return s;
+}
+}  // namespace synim
+
+namespace {
+
 #define SYNIM_CUDA(call)                                       \
     do {                                                       \
         cudaError_t e_ = (call);                               \

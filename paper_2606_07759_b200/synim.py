@@ -23,7 +23,7 @@ SLOPES_ND, SLOPES_GTILT = 0, 1
 EXPORTS = ("synim_compose_affine", "synim_create_geometry", "synim_num_rows", "synim_num_valid",
            "synim_row_offset", "synim_interaction_matrix", "synim_interaction_matrix_repaired", "synim_compute_bboxes",
            "synim_bbox_extent",
-           "synim_interaction_matrix_host", "synim_dictionary_host", "synim_destroy", "synim_last_error", "synim_version",
+           "synim_interaction_matrix_host", "synim_dictionary_host", "synim_projection_matrix", "synim_destroy", "synim_last_error", "synim_version",
            "synim_launch_count")
 
 PHYSICAL_FIELDS = ("shift_x", "shift_y", "rot_deg", "mag_x", "mag_y",
@@ -49,6 +49,11 @@ class Layer(ctypes.Structure):
     _fields_ = [("h_influence", ctypes.c_void_p), ("n_modes", ctypes.c_int32), ("ny", ctypes.c_int32),
                 ("nx", ctypes.c_int32), ("h_bbox", ctypes.c_void_p), ("affine", ctypes.POINTER(WfsAffine)),
                 ("h_out", ctypes.c_void_p)]
+
+
+class Component(ctypes.Structure):
+    _fields_ = [("d_cube", ctypes.c_void_p), ("n_modes", ctypes.c_int32), ("ny", ctypes.c_int32),
+                ("nx", ctypes.c_int32), ("maps", ctypes.POINTER(WfsAffine))]
 
 
 class SynimError(RuntimeError):
@@ -93,6 +98,9 @@ def lib() -> ctypes.CDLL:
         L.synim_interaction_matrix_host.argtypes = [vp, vp, i32, vp, ctypes.POINTER(WfsAffine), ctypes.c_int, vp, vp]
         L.synim_dictionary_host.restype = ctypes.c_int
         L.synim_dictionary_host.argtypes = [vp, ctypes.POINTER(Layer), i32, ctypes.c_int, vp]
+        L.synim_projection_matrix.restype = ctypes.c_int
+        L.synim_projection_matrix.argtypes = [ctypes.POINTER(Component), i32, ctypes.POINTER(Component), i32,
+                                              ctypes.POINTER(ctypes.c_double), vp, i32, ctypes.c_double, vp, i64, vp]
         L.synim_destroy.restype = None
         L.synim_destroy.argtypes = [vp]
         L.synim_last_error.restype = ctypes.c_char_p
@@ -368,6 +376,47 @@ def dictionary_host(geom: Geometry, layers: Sequence[dict], mode: int = SLOPES_N
     _check(lib().synim_dictionary_host(geom._h, arr, len(layers), int(mode), _stream_ptr(stream)))
     del keep
     return outs
+
+
+def projection_matrix(dm_cubes: Sequence, dm_maps: Sequence[Sequence[Sequence[float]]], layer_cube,
+                      layer_maps: Sequence[Sequence[float]], pupil, lam: float, weights: Optional[Sequence[float]] = None,
+                      out=None, stream=None):
+    """synim_projection_matrix: ``dm_cubes`` CUDA float32 cubes [n][ny][nx] of the mirrors with their
+    per-direction maps ``dm_maps[k][d]`` (a[6]); ``layer_cube`` / ``layer_maps`` likewise; ``pupil`` CUDA float32
+    [mp][mp].  Returns P_opt as a CUDA tensor viewed [n_layer_modes][ld] (row l = column l of the column-major
+    matrix: the projection of layer mode l onto all mirrors' modes)."""
+    import torch
+    n_dir = len(layer_maps)
+    comps = (Component * len(dm_cubes))()
+    keep = []
+    n_a = 0
+    for k, (cube, maps) in enumerate(zip(dm_cubes, dm_maps)):
+        assert cube.is_cuda and cube.dtype == torch.float32 and cube.is_contiguous() and cube.dim() == 3
+        assert len(maps) == n_dir
+        arr = _affine_array(maps, None)
+        keep.append(arr)
+        comps[k].d_cube, comps[k].n_modes, comps[k].ny, comps[k].nx = cube.data_ptr(), int(cube.shape[0]), int(cube.shape[1]), int(cube.shape[2])
+        comps[k].maps = ctypes.cast(arr, ctypes.POINTER(WfsAffine))
+        n_a += int(cube.shape[0])
+    assert layer_cube.is_cuda and layer_cube.dtype == torch.float32 and layer_cube.is_contiguous() and layer_cube.dim() == 3
+    lay = Component()
+    larr = _affine_array(layer_maps, None)
+    lay.d_cube, lay.n_modes, lay.ny, lay.nx = layer_cube.data_ptr(), int(layer_cube.shape[0]), int(layer_cube.shape[1]), int(layer_cube.shape[2])
+    lay.maps = ctypes.cast(larr, ctypes.POINTER(WfsAffine))
+    assert pupil.is_cuda and pupil.dtype == torch.float32 and pupil.is_contiguous() and pupil.dim() == 2 and pupil.shape[0] == pupil.shape[1]
+    n_l = int(layer_cube.shape[0])
+    if out is None:
+        out = torch.empty((n_l, n_a), dtype=torch.float32, device=layer_cube.device)
+    assert out.is_cuda and out.dtype == torch.float32 and out.dim() == 2 and out.stride(1) == 1 and out.shape[0] >= n_l
+    ld = int(out.stride(0)) if out.shape[0] > 1 else int(out.shape[1])
+    w = None
+    if weights is not None:
+        assert len(weights) == n_dir
+        w = (ctypes.c_double * n_dir)(*[float(v) for v in weights])
+    _check(lib().synim_projection_matrix(comps, len(dm_cubes), ctypes.byref(lay), n_dir, w, pupil.data_ptr(), int(pupil.shape[0]),
+                                         float(lam), out.data_ptr(), ld, _stream_ptr(stream)))
+    del keep, larr
+    return out
 
 
 def affines_of(workload) -> list:

@@ -690,6 +690,22 @@ __device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, 
         r_j0 = max(0, (int)floor(fmax(jmin, -lim)) - p.reach); r_j1 = min(W.M - 1, (int)ceil(fmin(jmax, lim)) + p.reach);
         r_i0 = max(0, (int)floor(fmax(imin, -lim)) - p.reach); r_i1 = min(W.M - 1, (int)ceil(fmin(imax, lim)) + p.reach);
         int4 win = make_int4(0, 0, 0, 0);
+        // A footprint that lies inside ONE subaperture (giant subapertures: config 4's 238-pixel NGS ones) whose pixel
+        // weights are all equal, or which is invalid, yields exactly nothing: the weighted sum of central differences
+        // telescopes to phi on the subaperture's two boundary column / row pairs (process_strip), where phi is 0 -- the
+        // D pixels that can be non-zero are uj0..uj1 x ui0..ui1, so phi vanishes outside uj0+1..uj1-1.  (The G-tilt sums
+        // read phi on the first / last valid pixels only: 0 as well.)  The column's zeros are already on their way.
+        {
+            const double uj0 = floor(fmax(jmin, -lim)) - p.reach, uj1 = ceil(fmin(jmax, lim)) + p.reach;
+            const double ui0 = floor(fmax(imin, -lim)) - p.reach, ui1 = ceil(fmin(imax, lim)) + p.reach;
+            if (uj0 >= 0.0 && ui0 >= 0.0 && uj1 <= (double)(W.M - 1) && ui1 <= (double)(W.M - 1)) {
+                const int sb = (int)uj0 / W.n_pix, sa = (int)ui0 / W.n_pix;
+                if ((int)uj1 / W.n_pix == sb && (int)ui1 / W.n_pix == sa) {
+                    const int c = __ldg(W.subap_row + sa * W.n_subap + sb);
+                    if (c < 0 || (c & kSubapGeneral) == 0) { r_j1 = r_j0 - 1; r_i1 = r_i0 - 1; }
+                }
+            }
+        }
         if (r_j1 >= r_j0 && r_i1 >= r_i0) {
             r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
             r_nb = r_j1 / W.n_pix - r_b0 + 1;

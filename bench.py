@@ -2,6 +2,7 @@
 """bench.py -- IM columns/s of the synthetic Shack-Hartmann interaction matrix on B200.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+                  [--slope-mode nd|gtilt] [--repair] [--dictionary MODES_PER_LAYER]
 
 A "step" is one pass of the whole hot path (S1-S4 of SURVEY.md sec. 8(a)) over one synthetic
 workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators x 6 LGS WFS =
@@ -18,6 +19,9 @@ workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators 
             (frac_datasheet)
   cpu_baseline  the float64 oracle, as it stands, on the host cores, on a bounded sample of modes
 
+--repair times synim_interaction_matrix_repaired (edge repair) on the config's modes cut by a
+source-frame mask; --dictionary M adds the 12-layer dictionary of PAPER.md:132 (M modes per layer) through
+synim_dictionary_host under config.dictionary.
 --impl reference times the oracle only (rank 0; other ranks exit).  N > 1: every rank holds its own
 workload of the same shape (independent problems, no data-path collective): weak scaling.
 """
@@ -352,19 +356,31 @@ def main():
     e2e = None
     if args.repair:
         args.no_e2e = True     # the host-buffer entry points have no repaired variant
+    e2e_error = None
     if not args.no_e2e:
         h_cube = torch.from_numpy(wl.cube).pin_memory()
         h_bbox = None if wl.bbox is None else torch.from_numpy(wl.bbox).pin_memory()
         h_out = torch.empty((wl.n_modes, geom.num_rows), dtype=torch.float32).pin_memory()
-        synim.interaction_matrix_host(geom, h_cube, h_bbox, affines, scales, out_host=h_out, stream=stream, mode=smode)
+
+        def host_step():
+            synim.interaction_matrix_host(geom, h_cube, h_bbox, affines, scales, out_host=h_out, stream=stream, mode=smode)
+        try:
+            host_step()
+        except Exception as exc:        # reported in the line; the device-resident numbers stand on their own
+            e2e_error = f"{type(exc).__name__}: {exc}"
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
-            synim.interaction_matrix_host(geom, h_cube, h_bbox, affines, scales, out_host=h_out, stream=stream, mode=smode)
-        torch.cuda.synchronize()
-        e2e_ms = 1e3 * (time.perf_counter() - t0) / args.e2e_steps
+        e2e_ms = 0.0
+        if e2e_error is None:
+            t0 = time.perf_counter()
+            try:
+                for _ in range(args.e2e_steps):
+                    host_step()
+            except Exception as exc:
+                e2e_error = f"{type(exc).__name__}: {exc}"
+            torch.cuda.synchronize()
+            e2e_ms = 1e3 * (time.perf_counter() - t0) / args.e2e_steps
         host_in = h_cube.numel() * 4 + (0 if h_bbox is None else h_bbox.numel() * 4)
         if h_bbox is None:
             h2d = host_in
@@ -375,11 +391,12 @@ def main():
             h2d = wl.n_modes * max(8, (bwm + 8) & ~3) * max(4, bhm + 2) * 4 + wl.n_modes * 24
         d2h = h_out.numel() * 4
         e2e_parity = None
-        if rank == 0:
+        if rank == 0 and e2e_error is None:
             got_h = h_out[torch.from_numpy(sel)].numpy().T.astype(np.float64)
             cmx = np.abs(ref).max(axis=0)
             e2e_parity = float((np.abs(got_h - got).max(axis=0) / np.maximum(cmx, 1e-30)).max())
-        e2e = (e2e_ms, h2d, d2h, host_in, e2e_parity)
+        if e2e_error is None:
+            e2e = (e2e_ms, h2d, d2h, host_in, e2e_parity)
 
     # the multi-layer dictionary of PAPER.md:132-138, end to end through host buffers (optional)
     dictionary = None
@@ -460,6 +477,8 @@ def main():
                            "host_input_bytes": e2e[3], "max_elementwise_vs_device_path": e2e[4],
                            "api": "synim_interaction_matrix_host (pinned host buffers; compact supports are packed "
                                   "on the host and only they cross the bus; chunks of modes pipelined: pack | H2D + kernel | D2H)"}
+        if e2e_error:
+            line["e2e"] = {"value": None, "unit": UNIT, "error": e2e_error}
         if world == 1 and not args.no_cpu_baseline:
             v, cores, desc = oracle_throughput(wl, 10.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}

@@ -270,66 +270,6 @@ def test_gtilt_estimator_on_the_gpu(S):
     assert_parity(gpu_im(S, wl, mode=S.SLOPES_GTILT, hint=False), O.interaction_matrix(wl, mode=O.GTILT), wl)
 
 
-def test_edge_repair_on_masked_modes(S):
-    """synim_interaction_matrix_repaired (PAPER.md:69-76) against the oracle's edge repair, on modes cut by a
-    source-frame mask: every BASELINE geometry (small subapertures under rotation, the cone effect with giant NGS
-    subapertures, dense Zernikes through the tile kernel), zonal and dense, with and without size hint / octagon."""
-    def check(wl, **kw):
-        ref = O.interaction_matrix(wl, repair_mask=wl.mask, threshold=kw.get("threshold", O.REPAIR_THRESHOLD))
-        raw = O.interaction_matrix(wl)
-        assert np.abs(ref - raw).max() > 1e-3 * np.abs(ref).max()      # the repair changes the matrix
-        assert_parity(gpu_im(S, wl, mask=wl.mask, **kw), ref, wl)
-    wl = W.masked(W.make_config(1), W.make_pupil(80, 80.0, 0.14))
-    check(wl)
-    check(wl, hint=False, octagon=False, ld_pad=3)
-    check(wl, use_bbox=False)                                          # dense: tiles of the WFS grid
-    check(W.masked(W.make_config(3, max_modes=48), W.make_pupil(480, 476.0, 0.28)))
-    check(W.masked(W.make_config(4, max_modes=24), W.make_pupil(600, 560.0, 0.1)))
-    check(W.masked(W.make_config(5, max_modes=2), W.make_pupil(480, 476.0, 0.28)))
-
-
-def test_edge_repair_soft_mask_thresholds_and_odd_sensors(S):
-    """A mask with soft (fractional) edges, holes and thin parts, sensors that look past the grid, strongly
-    (de)magnified ones, a single giant subaperture, one pixel per subaperture; the paper's threshold and 0.5."""
-    import scipy.ndimage as ndi
-    rng = np.random.default_rng(5)
-    ny, nx = 72, 88
-    cube = W.random_smooth_cube(4, ny, nx, 34)
-    blob = ndi.gaussian_filter(rng.normal(size=(ny, nx)), 4.0)
-    mask = np.clip(ndi.gaussian_filter((blob > np.quantile(blob, 0.3)).astype(float), 0.8) * 1.3, 0, 1).astype(np.float32)
-    pup = W.make_pupil(60, 60.0, 0.2)
-    sensors = []
-    for phys in (W.physical(shift_x=20.0, shift_y=-17.5, rot_deg=33.0), W.physical(mag_x=0.55, mag_y=0.6, rot_deg=-75.0),
-                 W.physical(mag_x=1.7, mag_y=1.5, shift_x=3.3, rot_deg=140.0)):
-        sensors.append(W.WfsInput(10, 6, pup, W.valid_subaps(pup, 10, 6), phys, slope_scale=1.7))
-    sensors.append(W.WfsInput(1, 44, np.ones((44, 44), np.float32), np.ones((1, 1), np.uint8),
-                              W.physical(rot_deg=5.0, mag_x=1.1, mag_y=1.1)))
-    p1 = W.make_pupil(40, 40.0, 0.0)
-    sensors.append(W.WfsInput(40, 1, p1, W.valid_subaps(p1, 40, 1), W.physical(rot_deg=-20.0, shift_x=1.5)))
-    wl = W.masked(W.Workload("soft mask", 0, ny, nx, cube, None, sensors), mask)
-    for thr in (O.REPAIR_THRESHOLD, 0.5):
-        ref = O.interaction_matrix(wl, repair_mask=mask, threshold=thr)
-        wl.bbox = None
-        assert_parity(gpu_im(S, wl, mask=mask, threshold=thr), ref, wl)
-        wl.bbox = W.tight_bboxes(wl.cube)
-        assert_parity(gpu_im(S, wl, mask=mask, threshold=thr), ref, wl)
-
-
-def test_edge_repair_argument_errors(S):
-    import torch
-    wl = W.masked(W.make_config(1, max_modes=4), W.make_pupil(80, 80.0, 0.14))
-    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
-    cube = torch.from_numpy(wl.cube).cuda()
-    mask = torch.from_numpy(wl.mask).cuda()
-    for thr in (0.0, 1.5, float("nan")):
-        with pytest.raises(S.SynimError) as e:
-            S.interaction_matrix(geom, cube, None, S.affines_of(wl), repair_mask=mask, threshold=thr)
-        assert e.value.status == S.ERR_INVALID_ARG
-    with pytest.raises(ValueError):
-        S.interaction_matrix(geom, cube, None, S.affines_of(wl), repair_mask=mask, mode=S.SLOPES_GTILT)
-    geom.destroy()
-
-
 def test_dense_path_on_zonal_cube_equals_bbox_path(S):
     """bbox = NULL must give the same matrix as the tile-skipping path (skipping is exact, R15)."""
     wl = W.make_config(1, max_modes=24)
@@ -616,3 +556,63 @@ def test_mode_ranges_through_the_library_concatenate_to_the_unsharded_matrix(S):
             assert torch.equal(out, whole)
         geom.destroy()
     assert_parity(whole.cpu().numpy().T.copy(), O.interaction_matrix(wl), wl)
+
+
+def test_edge_repair_on_masked_modes(S):
+    """synim_interaction_matrix_repaired (PAPER.md:69-76) against the oracle's edge repair, on modes cut by a
+    source-frame mask: every BASELINE geometry (small subapertures under rotation, the cone effect with giant NGS
+    subapertures, dense Zernikes through the tile kernel), zonal and dense, with and without size hint / octagon."""
+    def check(wl, **kw):
+        ref = O.interaction_matrix(wl, repair_mask=wl.mask, threshold=kw.get("threshold", O.REPAIR_THRESHOLD))
+        raw = O.interaction_matrix(wl)
+        assert np.abs(ref - raw).max() > 1e-3 * np.abs(ref).max()      # the repair changes the matrix
+        assert_parity(gpu_im(S, wl, mask=wl.mask, **kw), ref, wl)
+    wl = W.masked(W.make_config(1), W.make_pupil(80, 80.0, 0.14))
+    check(wl)
+    check(wl, hint=False, octagon=False, ld_pad=3)
+    check(wl, use_bbox=False)                                          # dense: tiles of the WFS grid
+    check(W.masked(W.make_config(3, max_modes=48), W.make_pupil(480, 476.0, 0.28)))
+    check(W.masked(W.make_config(4, max_modes=24), W.make_pupil(600, 560.0, 0.1)))
+    check(W.masked(W.make_config(5, max_modes=2), W.make_pupil(480, 476.0, 0.28)))
+
+
+def test_edge_repair_soft_mask_thresholds_and_odd_sensors(S):
+    """A mask with soft (fractional) edges, holes and thin parts, sensors that look past the grid, strongly
+    (de)magnified ones, a single giant subaperture, one pixel per subaperture; the paper's threshold and 0.5."""
+    import scipy.ndimage as ndi
+    rng = np.random.default_rng(5)
+    ny, nx = 72, 88
+    cube = W.random_smooth_cube(4, ny, nx, 34)
+    blob = ndi.gaussian_filter(rng.normal(size=(ny, nx)), 4.0)
+    mask = np.clip(ndi.gaussian_filter((blob > np.quantile(blob, 0.3)).astype(float), 0.8) * 1.3, 0, 1).astype(np.float32)
+    pup = W.make_pupil(60, 60.0, 0.2)
+    sensors = []
+    for phys in (W.physical(shift_x=20.0, shift_y=-17.5, rot_deg=33.0), W.physical(mag_x=0.55, mag_y=0.6, rot_deg=-75.0),
+                 W.physical(mag_x=1.7, mag_y=1.5, shift_x=3.3, rot_deg=140.0)):
+        sensors.append(W.WfsInput(10, 6, pup, W.valid_subaps(pup, 10, 6), phys, slope_scale=1.7))
+    sensors.append(W.WfsInput(1, 44, np.ones((44, 44), np.float32), np.ones((1, 1), np.uint8),
+                              W.physical(rot_deg=5.0, mag_x=1.1, mag_y=1.1)))
+    p1 = W.make_pupil(40, 40.0, 0.0)
+    sensors.append(W.WfsInput(40, 1, p1, W.valid_subaps(p1, 40, 1), W.physical(rot_deg=-20.0, shift_x=1.5)))
+    wl = W.masked(W.Workload("soft mask", 0, ny, nx, cube, None, sensors), mask)
+    for thr in (O.REPAIR_THRESHOLD, 0.5):
+        ref = O.interaction_matrix(wl, repair_mask=mask, threshold=thr)
+        wl.bbox = None
+        assert_parity(gpu_im(S, wl, mask=mask, threshold=thr), ref, wl)
+        wl.bbox = W.tight_bboxes(wl.cube)
+        assert_parity(gpu_im(S, wl, mask=mask, threshold=thr), ref, wl)
+
+
+def test_edge_repair_argument_errors(S):
+    import torch
+    wl = W.masked(W.make_config(1, max_modes=4), W.make_pupil(80, 80.0, 0.14))
+    geom = S.create_geometry(wl.ny, wl.nx, wl.wfs)
+    cube = torch.from_numpy(wl.cube).cuda()
+    mask = torch.from_numpy(wl.mask).cuda()
+    for thr in (0.0, 1.5, float("nan")):
+        with pytest.raises(S.SynimError) as e:
+            S.interaction_matrix(geom, cube, None, S.affines_of(wl), repair_mask=mask, threshold=thr)
+        assert e.value.status == S.ERR_INVALID_ARG
+    with pytest.raises(ValueError):
+        S.interaction_matrix(geom, cube, None, S.affines_of(wl), repair_mask=mask, mode=S.SLOPES_GTILT)
+    geom.destroy()

@@ -604,7 +604,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         for (int w = 0; w < nw; ++w) p.wfs[w] = dev[w0 + w];
         if (dense && dev[w0].spb > 0) {
             // two CTAs per SM: half the SM's shared memory less the per-CTA reserve and the static part
-            const size_t budget = (synim::max_dynamic_smem() + 1024) / 2 - 2048 - 8192;   // (8 KB: the warps' scratch)
+            const size_t budget = (synim::max_dynamic_smem() + 1024) / 2 - 2048 - (size_t)synim::kTileScratchBytesPerCta;   // (less the warps' scratch)
             bool fits = true;
             int tiles = 0, box_floats = 0, tab = 0;
             for (int w = 0; w < nw && fits; ++w) {

@@ -16,6 +16,10 @@ constexpr int kStripMaxCols = 30;      // D columns of a strip (one per lane, pl
 // them set: a ring pixel), bits 5..8 whether the next pixel P2 in that direction is one too.
 constexpr int kRepairCore = 1, kRepairP1Shift = 1, kRepairP2Shift = 5, kRepairRingMask = 0x1e;
 constexpr int kRepairReach = 2;        // a restored pixel reads up to two pixels away
+// tile kernel: per-warp scratch in which the lanes' partial sums of kEdgeBatch edge-sum units wait to be combined:
+// per unit 33 floats of column sums, 33 of row-pair differences, 66 of packed interior samples
+constexpr int kTileWarpsPerCta = 4, kEdgeBatch = 8, kEdgeSlotFloats = 33 + 33 + 66;
+constexpr int kTileScratchBytesPerCta = kTileWarpsPerCta * kEdgeBatch * kEdgeSlotFloats * 4;
 
 // One sensor as the kernel sees it.  All coordinates are ABSOLUTE pixel indices: WFS pixel (i, j)
 // (row, column) samples the source grid at

@@ -47,6 +47,9 @@ namespace {
 #ifndef SYNIM_STRIP_UNROLL
 #define SYNIM_STRIP_UNROLL 1   // unrolling of the row loop
 #endif
+#ifndef SYNIM_TILE_PACKED_EDGES
+#define SYNIM_TILE_PACKED_EDGES 1    // 0: the tile kernel samples every pixel of an edge-sum unit (comparisons)
+#endif
 #ifndef SYNIM_TILE_BATCHED_EDGES
 #define SYNIM_TILE_BATCHED_EDGES 1   // 0: the tile kernel combines the lanes of every edge-sum unit with shuffles (comparisons)
 #endif
@@ -61,7 +64,6 @@ static_assert(2 * kStripRows <= kWmapPadRows, "weight look-ahead runs past the r
 constexpr int kStripCols = kStripMaxCols;     // D columns per strip: lanes 1..30, halo on lanes 0 and 31
 constexpr float kMagicFloor = 12582912.0f;   // 1.5 * 2^23: fadd.rm(x, magic) = magic + floor(x), |x| < 2^22
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kEdgeBatch = 8;                // tile kernel: units whose lane sums are combined in one go (per-warp scratch)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -259,6 +261,29 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // source pixel, folded into the address base) and counted from their first row: |col|, |row| and rf stay below
     // ~40, so the float32 roundings of the base, of the product a1*rf and of the sum stay near 2e-6 pixels however
     // tall the strip is.  rr0 .. rr1: the phi rows (counted from i0-1) sampled until the next call.
+    // Packed interior samples of edge-sum units (kTile): the telescoped sums need phi on the first and last row of a
+    // unit in every column, but on its n-2 interior rows only in the boundary columns of the subapertures (their first
+    // and last column, and the strip's two halo columns): ncol = 2*nsb + 2 columns.  Those (n-2)*ncol samples are
+    // packed over the lanes, at most two per lane: lane l takes samples q = l and q = 32 + l, sample q being interior
+    // row 1 + q / ncol of boundary column q % ncol.  pj / pk: that sample's pixel column and row inside the unit.
+    constexpr bool kPacked = kTile && kEdge && SYNIM_TILE_PACKED_EDGES != 0;
+    const int p_nsb = kPacked ? div_npx(nC, W.n_pix, W.npx_magic) : 0, p_ncol = 2 * p_nsb + 2;
+    const int p_total = (W.n_pix - 2) * p_ncol;
+    const bool packed_ok = kPacked && W.n_pix >= 3 && p_total <= 64;
+    int pj[2] = {0, 0}, pk[2] = {0, 0};
+    bool pv[2] = {false, false};
+    float bcP[2] = {0.f, 0.f}, brP[2] = {0.f, 0.f};
+    if (packed_ok) {
+#pragma unroll
+        for (int s2 = 0; s2 < 2; ++s2) {
+            const int q = s2 * 32 + lane;
+            pv[s2] = q < p_total;
+            const int kr = q / p_ncol, kc = q - kr * p_ncol;
+            const int b = (kc - 1) >> 1, side = (kc - 1) & 1;
+            const int ln = kc == 0 ? 0 : (kc == p_ncol - 1 ? nC + 1 : 1 + b * W.n_pix + side * (W.n_pix - 1));
+            pj[s2] = jA - 1 + ln; pk[s2] = kr + 1;
+        }
+    }
     auto rebase = [&](int rr0, int rr1) {
         const double jm = (double)jA + 0.5 * (double)nC, im = (double)(i0 - 1) + 0.5 * (double)(rr0 + rr1);
         const int xc = __double2int_rn(W.fwd[0] * jm + W.fwd[1] * im + W.fwd[2] - (double)cb.x0);
@@ -268,6 +293,14 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
         br = (float)(W.fwd[3] * jl + W.fwd[4] * ib + W.fwd[5] - (double)(cb.y0 + yc));
         cbase = cb.base + (uint32_t)(yc * cb.pitch + xc) * 4u - addr_bias;
         roff = rr0;
+        if (packed_ok) {   // the packed samples' bases: pk rows below the unit's first row (whose rf is passed), column pj
+#pragma unroll
+            for (int s2 = 0; s2 < 2; ++s2) {
+                const double pjd = (double)pj[s2], pid = ib + (double)pk[s2];
+                bcP[s2] = (float)(W.fwd[0] * pjd + W.fwd[1] * pid + W.fwd[2] - (double)(cb.x0 + xc));
+                brP[s2] = (float)(W.fwd[3] * pjd + W.fwd[4] * pid + W.fwd[5] - (double)(cb.y0 + yc));
+            }
+        }
     };
     const float a1 = (float)W.fwd[1], a4 = (float)W.fwd[4];
     const float cwf = (float)cb.cw, chf = (float)cb.ch;
@@ -562,6 +595,63 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
                 }
             }
             if (rem > 0 && d_end == d_hi) { flush_general(sx, sy); rem = 0; }   // the walk ended inside a unit
+        } else if (packed_ok) {
+            // Edge-sum units of a tile, boundary samples only (see kPacked above): per unit two full rows (its last row
+            // and the next unit's first) and at most two packed samples per lane instead of n full rows.  Parked per
+            // unit in the warp's scratch: csp = phi[first row] + phi[last row] of the lane's column, v = the difference
+            // of the two row pairs, pk = the packed samples; combined kEdgeBatch units at a time.
+            const int nu = (d_end - d + 1) / npx;
+            const int nsb = p_nsb, ncol = p_ncol;
+            constexpr uint32_t kSlot4 = (uint32_t)kEdgeSlotFloats * 4u;
+            auto packed_phase2 = [&](int a_start, int cnt) {
+                __syncwarp();
+                for (int t = lane; t < cnt * nsb; t += 32) {
+                    const int uu = t / nsb, sb = t - uu * nsb;
+                    const uint32_t base = scr + (uint32_t)uu * kSlot4;
+                    const uint32_t c0 = base + (uint32_t)(sb * npx) * 4u, c2 = base + (uint32_t)((sb + 1) * npx) * 4u;
+                    float s_lo = lds_f32(c0) + lds_f32(c0 + 4u), s_hi = lds_f32(c2) + lds_f32(c2 + 4u);
+                    uint32_t pr = base + (uint32_t)(66 + 2 * sb) * 4u;   // interior row 1, boundary column 2*sb
+                    for (int k = 0; k < npx - 2; ++k, pr += (uint32_t)ncol * 4u) {
+                        s_lo += lds_f32(pr) + lds_f32(pr + 4u);
+                        s_hi += lds_f32(pr + 8u) + lds_f32(pr + 12u);
+                    }
+                    const uint32_t rv = base + (uint32_t)(33 + 1 + sb * npx) * 4u;
+                    float sy = lds_f32(rv);
+                    for (int k = 1; k < npx; ++k) sy += lds_f32(rv + (uint32_t)k * 4u);
+                    const uint32_t te = tab + (uint32_t)((a_start + uu - a0) * nb + (seg_first - b0) + sb) * 8u;
+#ifdef SYNIM_CHECKS
+                    if (te < tab || te + 8u > tab + (uint32_t)W.tab_cap * 4u) __trap();
+#endif
+                    sts_f32(te, (s_hi - s_lo) * wu);
+                    sts_f32(te + 4u, sy * wu);
+                }
+                __syncwarp();
+            };
+            float pairt = pmA + pmB, carry = pmB;   // phi[i0-1] + phi[i0] and phi[i0] of the current unit
+            int slot = 0, a_batch = a_cur;
+            int rr = d + 1;   // phi row after the unit's first (counted from i0-1): rf is its re-based float
+            for (int uu = 0; uu < nu; ++uu, rr += npx) {
+                if (uu != 0 && (uu & (kRebaseUnits - 1)) == 0) {
+                    rebase(rr, min(d_end + 1, rr + rebase_rows));
+                    rf = 0.0f;
+                }
+                const float rfu = rf - 1.0f;   // the unit's first row
+                const float fl = sample(rfu + (float)(npx - 1)), fn = sample(rfu + (float)npx);
+                float k0 = 0.0f, k1 = 0.0f;
+                if (pv[0]) k0 = sample_xy(fmaf(a1, rfu, bcP[0]), fmaf(a4, rfu, brP[0]));
+                if (pv[1]) k1 = sample_xy(fmaf(a1, rfu, bcP[1]), fmaf(a4, rfu, brP[1]));
+                rf += (float)npx;
+                const float pairb = fl + fn;
+                const uint32_t sl = scr + (uint32_t)slot * kSlot4 + (uint32_t)lane * 4u;
+                sts_f32(sl, carry + fl);
+                sts_f32(sl + 33u * 4u, pairb - pairt);
+                sts_f32(sl + 66u * 4u, k0);
+                sts_f32(sl + 98u * 4u, k1);
+                pairt = pairb; carry = fn;
+                if (++slot == kEdgeBatch) { packed_phase2(a_batch, slot); a_batch += slot; slot = 0; }
+            }
+            if (slot) packed_phase2(a_batch, slot);
+            a_cur += nu; tent += tstep * (uint32_t)nu;
         } else if (kTile && SYNIM_TILE_BATCHED_EDGES != 0) {
             // Edge-sum units of a tile: whole units, four rows in flight.  Per unit and lane only the column sum cs
             // and the difference v of the two row pairs are formed; they are parked in the warp's scratch
@@ -939,11 +1029,8 @@ __global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : SYNIM_STRIP_MINB)
 // CTA, with plain streaming stores: no memset, no atomics.  CTAs are ordered mode-major, so a mode's image is read
 // from HBM once and served from L2 to the other tiles and sensors (the cube is fetched once for all
 // WFS).  Units of invalid subapertures (outside the pupil) are skipped.
-#ifndef SYNIM_TILE_WARPS
-#define SYNIM_TILE_WARPS 4
-#endif
-constexpr int kTileWarps = SYNIM_TILE_WARPS, kTileThreads = 32 * kTileWarps;
-constexpr int kTileScratchFloats = 2 * kEdgeBatch * 33;   // per warp: cs and v of kEdgeBatch units, one float per lane (+1 pad)
+constexpr int kTileWarps = kTileWarpsPerCta, kTileThreads = 32 * kTileWarps;
+constexpr int kTileScratchFloats = kEdgeBatch * kEdgeSlotFloats;   // per warp
 
 __device__ __forceinline__ void tma_load_box_plain(void *dst, const void *map, uint64_t *bar, int x, int y, int z)
 {

@@ -16,7 +16,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "synim_oracle.c")
-_LIB = os.path.join(_HERE, "liboracle.so")
+#: SYNIM_ORACLE_LIB points the front end at another build of the same source (the sanitizer run of the tests)
+_LIB = os.environ.get("SYNIM_ORACLE_LIB") or os.path.join(_HERE, "liboracle.so")
 
 ND, GTILT = 0, 1
 
@@ -29,6 +30,8 @@ _FIELDS = ("shift_x", "shift_y", "rot_deg", "mag_x", "mag_y",
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain C, OpenMP over modes)."""
+    if os.environ.get("SYNIM_ORACLE_LIB"):
+        return _LIB
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
                                "-o", _LIB, _SRC, "-lm"])

@@ -424,3 +424,36 @@ def test_zernike_modes_are_orthonormal_low_order_and_bounded_high_order():
     # (inside the disc only: rho is clamped to 1 outside it)
     assert W.noll_to_nm(2) == (1, 1)
     assert np.allclose((cube[0] / cube[0, 64, 100] * x[64, 100])[m], x[m], rtol=1e-5, atol=1e-4)
+
+
+def test_oracle_runs_clean_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """the oracle's C source built with -fsanitize=address,undefined runs every entry point
+    (numerical derivative, G-tilt, edge repair, halo resampling, composition) on odd-sized inputs whose samples leave
+    the source grid, in a subprocess; any out-of-bounds access or undefined operation aborts it."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    lib = str(tmp_path / "liboracle_san.so")
+    subprocess.check_call(["gcc", "-O1", "-g", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-fsanitize=address,undefined",
+                           "-fno-sanitize-recover=undefined", "-o", lib, os.path.join(root, "oracle", "synim_oracle.c"), "-lm"])
+    asan = subprocess.check_output(["gcc", "-print-file-name=libasan.so"], text=True).strip()
+    code = (
+        "import numpy as np\n"
+        "from oracle import oracle as O\n"
+        "from paper_2606_07759_b200 import workloads as W\n"
+        "rng = np.random.default_rng(0)\n"
+        "cube = rng.normal(size=(3, 20, 28)).astype(np.float32)\n"
+        "pup = W.make_pupil(21, 21.0, 0.2)\n"
+        "val = W.valid_subaps(pup, 3, 7)\n"
+        "a = [0.7, 0.9, 6.0, -0.9, 0.7, -5.0]\n"
+        "for mode in (O.ND, O.GTILT):\n"
+        "    assert np.isfinite(O.slopes_wfs(cube, pup, 3, 7, val, a, 1.5, mode, modes=[2, 0], n_threads=2)).all()\n"
+        "mask = (rng.uniform(size=(20, 28)) > 0.2).astype(np.float32)\n"
+        "assert np.isfinite(O.slopes_wfs_repair(cube, mask, pup, 3, 7, val, a)).all()\n"
+        "O.repair_screen(cube[0], mask, 21, a); O.resample(cube[1], 21, a, halo=True)\n"
+        "O.compose_affine(W.physical(rot_deg=33.0, dm_height_m=17000.0, gs_range_m=90000.0, gs_theta_arcsec=45.0, src_pixel_pitch_m=0.08))\n"
+        "print('clean')\n")
+    env = dict(os.environ, SYNIM_ORACLE_LIB=lib, LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0", PYTHONPATH=root)
+    out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, cwd=root, timeout=300)
+    assert out.returncode == 0 and "clean" in out.stdout, out.stderr[-2000:]

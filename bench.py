@@ -22,6 +22,8 @@ workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators 
 --repair times synim_interaction_matrix_repaired (edge repair) on the config's modes cut by a
 source-frame mask; --dictionary M adds the 12-layer dictionary of PAPER.md:132 (M modes per layer) through
 synim_dictionary_host under config.dictionary.
+--extra (default "2,4,5,3r,3g"): at N=1 the line also carries, under config.other_configs, short device-resident runs
+of the other configurations, each in its own process.
 --impl reference times the oracle only (rank 0; other ranks exit).  N > 1: every rank holds its own
 workload of the same shape (independent problems, no data-path collective): weak scaling.
 """
@@ -157,6 +159,41 @@ def config_dict(wl, extra=None):
     return d
 
 
+def other_configs(spec: str) -> dict:
+    """Short device-resident runs of the other configurations (cold-L2 protocol, 10 steps), one process each so that
+    nothing they do can take the headline run down; what the line keeps of each: step time, columns/s, roofline
+    fractions, the dominant kernel and the parity spot check."""
+    out = {}
+    for tag in [t.strip() for t in spec.split(",") if t.strip()]:
+        cfg = tag.rstrip("rg")
+        if cfg not in ("1", "2", "3", "4", "5"):
+            out[tag] = {"error": "unknown tag"}
+            continue
+        cmd = [sys.executable, os.path.abspath(__file__), "--config", cfg, "--steps", "10", "--warmup", "3", "--no-e2e",
+               "--no-cpu-baseline", "--parity-modes", "32", "--extra", "none"]
+        if tag.endswith("r"):
+            cmd.append("--repair")
+        if tag.endswith("g"):
+            cmd += ["--slope-mode", "gtilt"]
+        try:
+            res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+            last = [ln for ln in res.stdout.strip().splitlines() if ln.startswith("{")]
+            if res.returncode != 0 or not last:
+                out[tag] = {"error": (res.stderr or res.stdout)[-400:]}
+                continue
+            d = json.loads(last[-1])
+            out[tag] = {"workload": d["config"]["workload"], "columns": d["config"]["columns"], "ms_per_step": d["ms_per_step"],
+                        "cold_ms_min_med_max": d["config"]["cold_ms_min_med_max"], "warm_ms_per_step": d["config"]["warm_ms_per_step"],
+                        "columns_per_s": d["value"], "frac": d["roofline"]["frac"], "frac_datasheet": d["roofline"]["frac_datasheet"],
+                        "algorithmic_bytes": d["roofline"]["algorithmic_bytes"]["total"], "kernel": d["roofline"]["kernel"],
+                        "gpu_launches": d["gpu_launches"], "parity_spot_check": d["parity_spot_check"],
+                        "clocks": d["clocks"], "slope_mode": d["config"].get("slope_mode"),
+                        "edge_repair": d["config"].get("edge_repair")}
+        except Exception as exc:
+            out[tag] = {"error": f"{type(exc).__name__}: {exc}"}
+    return out
+
+
 def run_reference(args, rank: int):
     if rank != 0:
         return
@@ -196,6 +233,10 @@ def main():
     ap.add_argument("--dictionary", type=int, default=0, metavar="MODES_PER_LAYER",
                     help="also run the 12-layer dictionary of PAPER.md:132 (workloads.make_dictionary, this many modes per "
                          "layer) through synim_dictionary_host and report it under config.dictionary")
+    ap.add_argument("--extra", default="2,4,5,3r,3g",
+                    help="at N=1, after the timed run: short device-resident runs of these other configurations, each in its "
+                         "own process, reported under config.other_configs ('3r' = config 3 with edge repair, '3g' = config 3 "
+                         "with the G-tilt estimator; 'none' to skip)")
     ap.add_argument("--slope-mode", default="nd", choices=["nd", "gtilt"],
                     help="nd = the paper's numerical-derivative engine (the metric); gtilt = the comparison estimator")
     args = ap.parse_args()
@@ -465,7 +506,7 @@ def main():
                              "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of the committed ncu capture "
                                                "(profiles/dram_traffic.csv), not measured in this run",
                              "peak_source": peak_src, "algorithmic_bytes": ab,
-                             "kernel": synim.hot_kernel_name(dense=wl.bbox is None), "kernel_ms": kernel_ms,
+                             "kernel": synim.hot_kernel_name(wl.bbox is None, args.slope_mode == "gtilt", args.repair), "kernel_ms": kernel_ms,
                              "warm_frac": ab["total"] / (float(warm.mean()) * 1e-3) / 1e9 / peak},
                 "clocks": clocks, "gpu_launches": 2 * args.steps * launches_per_step,
                 "gpu_launches_note": f"{launches_per_step} launch(es) of this library's kernels per step (counted by the library), "
@@ -479,6 +520,8 @@ def main():
                                   "on the host and only they cross the bus; chunks of modes pipelined: pack | H2D + kernel | D2H)"}
         if e2e_error:
             line["e2e"] = {"value": None, "unit": UNIT, "error": e2e_error}
+        if world == 1 and args.extra.strip().lower() != "none":
+            line["config"]["other_configs"] = other_configs(args.extra)
         if world == 1 and not args.no_cpu_baseline:
             v, cores, desc = oracle_throughput(wl, 10.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}

@@ -127,9 +127,12 @@ def launch_count() -> int:
     return int(lib().synim_launch_count())
 
 
-def hot_kernel_name(dense: bool) -> str:
+def hot_kernel_name(dense: bool, gtilt: bool = False, repair: bool = False) -> str:
     """Name of the kernel that dominates a step (for reports; the launch lists under profiles/ show it)."""
-    return "synim_tile_kernel<false> (dense modes: tiles of the WFS grid)" if dense else "synim_strip_kernel<false, true>"
+    g, r = ("true" if gtilt else "false"), ("true" if repair else "false")
+    if dense:
+        return f"synim_tile_kernel<{g}, {r}> (dense modes: tiles of the WFS grid)"
+    return f"synim_strip_kernel<{g}, true, {r}>"
 
 
 def last_error() -> str:

@@ -310,9 +310,12 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // row lies between its two end points, and each limit is a half-plane
     // (kRepair: a restored pixel reads up to kRepairReach pixels away, along its row or its column)
     const float a0f = (float)W.fwd[0], a3f = (float)W.fwd[3];
-    const float reachf = kRepair ? (float)kRepairReach : 0.0f;
-    const float bcL = __shfl_sync(kFull, bc, 0) - reachf * a0f, brL = __shfl_sync(kFull, br, 0) - reachf * a3f;
-    const float bcR = __shfl_sync(kFull, bc, nC + 1) + reachf * a0f, brR = __shfl_sync(kFull, br, nC + 1) + reachf * a3f;
+    float bcL = __shfl_sync(kFull, bc, 0), brL = __shfl_sync(kFull, br, 0);
+    float bcR = __shfl_sync(kFull, bc, nC + 1), brR = __shfl_sync(kFull, br, nC + 1);
+    if (kRepair) {
+        bcL -= (float)kRepairReach * a0f; brL -= (float)kRepairReach * a3f;
+        bcR += (float)kRepairReach * a0f; brR += (float)kRepairReach * a3f;
+    }
     int first = 0x7fffffff, last = -1;
     if (kTile) { first = 0; last = nR + 1; }
     for (int g = 0; !kTile && g < nR + 2; g += 32) {
@@ -601,7 +604,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
             // unit in the warp's scratch: csp = phi[first row] + phi[last row] of the lane's column, v = the difference
             // of the two row pairs, pk = the packed samples; combined kEdgeBatch units at a time.
             const int nu = (d_end - d + 1) / npx;
-            const int nsb = p_nsb, ncol = p_ncol;
+            const int nsb = max(p_nsb, 1), ncol = p_ncol;   // (p_nsb >= 1 here; the max keeps dead instantiations quiet)
             constexpr uint32_t kSlot4 = (uint32_t)kEdgeSlotFloats * 4u;
             auto packed_phase2 = [&](int a_start, int cnt) {
                 __syncwarp();

@@ -176,7 +176,8 @@ def other_configs(spec: str) -> dict:
         if tag.endswith("g"):
             cmd += ["--slope-mode", "gtilt"]
         try:
-            res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+            res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT,
+                                 env=dict(os.environ, SYNIM_BENCH_CHILD="1"))
             last = [ln for ln in res.stdout.strip().splitlines() if ln.startswith("{")]
             if res.returncode != 0 or not last:
                 out[tag] = {"error": (res.stderr or res.stdout)[-400:]}
@@ -259,7 +260,7 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    if rank == 0:
+    if rank == 0 and not os.environ.get("SYNIM_BENCH_CHILD"):      # (a child of other_configs: the parent has built it)
         build.build_library()
     if dist is not None:
         dist.barrier()

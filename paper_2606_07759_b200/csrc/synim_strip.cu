@@ -1,7 +1,14 @@
-// synim_strip.cu -- the interaction-matrix kernel for sm_100a (S1-S4 of SURVEY.md sec. 8(a)).
+// synim_strip.cu -- the interaction-matrix kernels for sm_100a (S1-S4 of SURVEY.md sec. 8(a)).
 //
-// Compact-support ("zonal") modes: one CTA per mode.  (Dense modes: the whole grid cut into pieces, several
-// CTAs per mode -- see the kernel; G-tilt instead of the numerical derivative -- see process_strip.)  The mode's support (its bbox plus the one-pixel ring a bilinear sample can still
+// Two kernels around one strip walker (process_strip):
+//   synim_strip_kernel  compact-support ("zonal") modes: one CTA per mode, all sensors -- described below;
+//   synim_tile_kernel   dense (modal) cubes: one CTA per (mode, sensor, tile of the WFS grid), output-stationary --
+//                       described above its definition.
+// Template flags: kGtilt (the G-tilt estimator instead of the numerical derivative), kAligned (strips hold whole
+// subaperture columns; edge-sum path on uniformly lit subapertures), kTile (the strip is a piece of a staged tile),
+// kRepair (edge repair) -- see process_strip.
+//
+// Zonal modes: the mode's support (its bbox plus the one-pixel ring a bilinear sample can still
 // touch) is staged ONCE in shared memory by a TMA 3-D box load (cp.async.bulk.tensor, out-of-range
 // elements zero-filled by the hardware = reading R4) and reused by every sensor of the batch
 // (the cube is fetched once for all WFS).  Each warp then takes "strips": 30 WFS pixel
@@ -15,11 +22,13 @@
 //   S3  D_y from registers, D_x from the two neighbouring lanes (shuffles), weighted by the
 //       precomputed 0.5*P/W_S map, summed down the rows of a subaperture in registers, across its
 //       columns with a segmented warp-shuffle reduction, and into a per-CTA shared table of
-//       (sensor, subaperture, axis) slopes,
+//       (sensor, subaperture, axis) slopes; on uniformly lit subapertures the sums telescope to the
+//       boundary rows and columns (edge-sum path: no stencil, no weights),
 //   S4  the column is written once: its zeros by plain 16-byte stores PACED through the sampling loop
 //       (one per thread per iteration), then the table's non-zero entries on top.
 // Rows of a strip that cannot touch the support are never sampled (exact: phi is 0 there, R15).
-// phi is never written anywhere.
+// phi is never written anywhere.  A support larger than the staged box (no size hint, > 128 px, or dense
+// modes seen by subapertures wider than a strip) is split into pieces whose slopes add up (global RED).
 //
 // Measured on B200, round 1 (profiles/README.md): FFMA2/FADD2 occupy the issue port for two cycles, so
 // packing pixel pairs into f32x2 saves nothing; LDS and SHFL each run at about one warp instruction

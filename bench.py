@@ -22,7 +22,7 @@ workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators 
 --repair times synim_interaction_matrix_repaired (edge repair) on the config's modes cut by a
 source-frame mask; --dictionary M adds the 12-layer dictionary of PAPER.md:132 (M modes per layer) through
 synim_dictionary_host under config.dictionary.
---extra (default "2,4,5,3r,3g"): at N=1 the line also carries, under config.other_configs, short device-resident runs
+--extra (default "2,4,5,3r,3g,3p"): at N=1 the line also carries, under config.other_configs, short device-resident runs
 of the other configurations, each in its own process.
 --impl reference times the oracle only (rank 0; other ranks exit).  N > 1: every rank holds its own
 workload of the same shape (independent problems, no data-path collective): weak scaling.
@@ -165,7 +165,7 @@ def other_configs(spec: str) -> dict:
     fractions, the dominant kernel and the parity spot check."""
     out = {}
     for tag in [t.strip() for t in spec.split(",") if t.strip()]:
-        cfg = tag.rstrip("rg")
+        cfg = tag.rstrip("rgp")
         if cfg not in ("1", "2", "3", "4", "5"):
             out[tag] = {"error": "unknown tag"}
             continue
@@ -175,9 +175,11 @@ def other_configs(spec: str) -> dict:
             cmd.append("--repair")
         if tag.endswith("g"):
             cmd += ["--slope-mode", "gtilt"]
+        env = dict(os.environ, SYNIM_BENCH_CHILD="1")
+        if tag.endswith("p"):
+            env["SYNIM_ZONAL_PACKED"] = "1"
         try:
-            res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT,
-                                 env=dict(os.environ, SYNIM_BENCH_CHILD="1"))
+            res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
             last = [ln for ln in res.stdout.strip().splitlines() if ln.startswith("{")]
             if res.returncode != 0 or not last:
                 out[tag] = {"error": (res.stderr or res.stdout)[-400:]}
@@ -189,7 +191,8 @@ def other_configs(spec: str) -> dict:
                         "algorithmic_bytes": d["roofline"]["algorithmic_bytes"]["total"], "kernel": d["roofline"]["kernel"],
                         "gpu_launches": d["gpu_launches"], "parity_spot_check": d["parity_spot_check"],
                         "clocks": d["clocks"], "slope_mode": d["config"].get("slope_mode"),
-                        "edge_repair": d["config"].get("edge_repair")}
+                        "edge_repair": d["config"].get("edge_repair"),
+                        "packed_zonal_walk": tag.endswith("p")}
         except Exception as exc:
             out[tag] = {"error": f"{type(exc).__name__}: {exc}"}
     return out
@@ -234,10 +237,11 @@ def main():
     ap.add_argument("--dictionary", type=int, default=0, metavar="MODES_PER_LAYER",
                     help="also run the 12-layer dictionary of PAPER.md:132 (workloads.make_dictionary, this many modes per "
                          "layer) through synim_dictionary_host and report it under config.dictionary")
-    ap.add_argument("--extra", default="2,4,5,3r,3g",
+    ap.add_argument("--extra", default="2,4,5,3r,3g,3p",
                     help="at N=1, after the timed run: short device-resident runs of these other configurations, each in its "
                          "own process, reported under config.other_configs ('3r' = config 3 with edge repair, '3g' = config 3 "
-                         "with the G-tilt estimator; 'none' to skip)")
+                         "with the G-tilt estimator, '3p' = config 3 through the opt-in packed zonal walk, SYNIM_ZONAL_PACKED=1; "
+                         "'none' to skip)")
     ap.add_argument("--slope-mode", default="nd", choices=["nd", "gtilt"],
                     help="nd = the paper's numerical-derivative engine (the metric); gtilt = the comparison estimator")
     args = ap.parse_args()

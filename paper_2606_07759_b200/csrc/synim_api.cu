@@ -657,6 +657,9 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         }
         p.patch_pitchf = (float)patch_pitch;
         p.patch_pitch = patch_pitch; p.patch_h = patch_h;
+        // opt-in until measured on hardware: the packed boundary-only walk for zonal modes
+        p.unit_rows = (!dense && !repair && mode == SYNIM_SLOPES_ND && dev[w0].spb > 0 && std::getenv("SYNIM_ZONAL_PACKED") &&
+                       std::atoi(std::getenv("SYNIM_ZONAL_PACKED")) != 0) ? 1 : 0;
         p.tab_floats = nw > 0 ? (dev[w0 + nw - 1].tab_off + dev[w0 + nw - 1].tab_cap + 3) & ~3 : 0;
         p.chunks = chunks;
         if (dense) {

@@ -68,6 +68,7 @@ struct ImParams {
     unsigned addr_bias;         // (bits of 1.5*2^23) << 2 mod 2^32, see process_strip
     int tab_floats;             // size of the CTA's slope table (multiple of 4)
     int tiles_total;            // tile kernel: tiles of one mode over all sensors of the launch
+    int unit_rows;              // 1: aligned sensors' footprints are rounded out to whole subaperture rows (packed zonal walk)
     int reach;                  // extra pixels around a tile / a footprint that a sample may touch: 0, or kRepairReach
     WfsDev wfs[kMaxWfsPerLaunch];
 };
@@ -81,6 +82,8 @@ struct alignas(64) TileMaps {
 // launchers; all asynchronous on `stream`, return the launch status.
 // The hot path (synim_strip.cu); tensor_map points at a host CUtensorMap over the cube with box
 // {patch_pitch, patch_h, 1}
+// (p.unit_rows selects the packed zonal walk: numerical derivative, aligned sensors, no repair; the launcher adds the
+// warps' scratch to smem_bytes)
 cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_bytes, bool gtilt, bool repair,
                          cudaStream_t stream);
 // Dense modes over sensors whose subapertures fit a strip: one CTA per (mode, sensor, tile of the WFS grid);

@@ -243,12 +243,16 @@ __device__ __forceinline__ int div_npx(int x, int npx, unsigned magic) { return 
 // bilinear sample of its own, taken by the lane that needs it), 0 elsewhere -- per the pixel classes W.rcode that
 // repair_maps built for this call; W.wmap then holds 0.5*P*core/sum(P*core) and W.subap_row flags as general every
 // subaperture that is not core throughout, so the edge-sum path only ever sees unrepaired pixels.
-template <bool kGtilt, bool kAligned, bool kTile, bool kRepair>
+// kWalk: 0 = the classic walk of a footprint (rows pruned to the support, partial units at either end); 1 = kTile;
+// 2 = a zonal footprint whose rows were rounded out to whole units (ImParams::unit_rows), so that its edge-sum units can
+// take the packed boundary-only path of the tile kernel (opt-in, SYNIM_ZONAL_PACKED=1: not the default until measured).
+template <bool kGtilt, bool kAligned, int kWalk, bool kRepair>
 __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, int jA, int nC, const CellBox &cb,
                                               uint32_t addr_bias, uint32_t tab, int a0, int b0, int nb, ZeroPacer &zp,
                                               uint32_t scr = 0u)
 {
-    static_assert(!kTile || kAligned, "tiles are made of aligned strips");
+    constexpr bool kTile = kWalk == 1, kWhole = kWalk != 0;   // kWhole: the walk consists of whole units
+    static_assert(!kWhole || kAligned, "whole-unit walks are made of aligned strips");
     static_assert(!kRepair || !kGtilt, "edge repair belongs to the numerical-derivative engine");
     constexpr bool kEdge = kAligned && !kGtilt && SYNIM_EDGE_SUM != 0;   // the edge-sum path exists
     constexpr int kRows = kStripRows;
@@ -275,7 +279,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // and last column, and the strip's two halo columns): ncol = 2*nsb + 2 columns.  Those (n-2)*ncol samples are
     // packed over the lanes, at most two per lane: lane l takes samples q = l and q = 32 + l, sample q being interior
     // row 1 + q / ncol of boundary column q % ncol.  pj / pk: that sample's pixel column and row inside the unit.
-    constexpr bool kPacked = kTile && kEdge && SYNIM_TILE_PACKED_EDGES != 0;
+    constexpr bool kPacked = kWhole && kEdge && SYNIM_TILE_PACKED_EDGES != 0;
     const int p_nsb = kPacked ? div_npx(nC, W.n_pix, W.npx_magic) : 0, p_ncol = 2 * p_nsb + 2;
     const int p_total = (W.n_pix - 2) * p_ncol;
     const bool packed_ok = kPacked && W.n_pix >= 3 && p_total <= 64;
@@ -291,6 +295,11 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
             const int b = (kc - 1) >> 1, side = (kc - 1) & 1;
             const int ln = kc == 0 ? 0 : (kc == p_ncol - 1 ? nC + 1 : 1 + b * W.n_pix + side * (W.n_pix - 1));
             pj[s2] = jA - 1 + ln; pk[s2] = kr + 1;
+            if (kWalk == 2) {   // (no re-basing in a zonal walk: relative to the staged box, once per strip)
+                const double pjd = (double)pj[s2], pid = (double)(i0 - 1 + pk[s2]);
+                bcP[s2] = (float)(W.fwd[0] * pjd + W.fwd[1] * pid + W.fwd[2] - (double)cb.x0);
+                brP[s2] = (float)(W.fwd[3] * pjd + W.fwd[4] * pid + W.fwd[5] - (double)cb.y0);
+            }
         }
     }
     auto rebase = [&](int rr0, int rr1) {
@@ -344,8 +353,12 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     }
     if (last < 0) return;
     const int row_reach = kRepair ? 1 + kRepairReach : 1;
-    const int d_lo = max(first - row_reach, 1), d_hi = min(last + row_reach, nR);   // D rows that can be non-zero
+    int d_lo = max(first - row_reach, 1), d_hi = min(last + row_reach, nR);   // D rows that can be non-zero
     if (d_hi < d_lo) return;
+    if (kWalk == 2) {   // whole units (the footprint starts and ends on unit boundaries; the rows added hold phi = 0)
+        d_lo = ((d_lo - 1) / W.n_pix) * W.n_pix + 1;
+        d_hi = min(((d_hi + W.n_pix - 1) / W.n_pix) * W.n_pix, nR);
+    }
 
     // segments of lanes that belong to one subaperture column
     const int npx = W.n_pix, n_subap = W.n_subap;
@@ -374,7 +387,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     // its unit; units beyond 32 are simply taken as general)
     // bit u of skipmask (kTile): none of the strip's subapertures of unit a_first+u is valid
     unsigned genmask = 0xffffffffu, skipmask = 0u;
-    if (kEdge || kTile) {
+    if (kEdge || kWhole) {
         const int bA = div_npx(jA, npx, W.npx_magic), nsb = div_npx(nC, npx, W.npx_magic);
         const int a_mine = a_first + lane;
         bool gflag = false, vflag = false;
@@ -388,7 +401,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
                 }
         }
         if (kEdge) genmask = __ballot_sync(kFull, gflag);
-        if (kTile) skipmask = __ballot_sync(kFull, a_mine < n_subap && !vflag);
+        if (kWhole) skipmask = __ballot_sync(kFull, a_mine < n_subap && !vflag);
         genmask &= ~skipmask;
     }
 
@@ -529,10 +542,10 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
     while (d <= d_hi) {
         // the segment: units of one kind from the current one on; D rows d .. d_end
         const int u = a_cur - a_first;
-        const bool skip = kTile && u < 32 && ((skipmask >> u) & 1u);
+        const bool skip = kWhole && u < 32 && ((skipmask >> u) & 1u);
         const bool gen = !skip && (!kEdge || u >= 32 || ((genmask >> u) & 1u));
         int d_end = d_hi;
-        if ((kEdge || kTile) && u < 32) {
+        if ((kEdge || kWhole) && u < 32) {
             const unsigned mine = skip ? skipmask : (gen ? genmask : ~(genmask | skipmask));
             const unsigned other = ~mine >> u;   // bit k: unit u+k is of another kind
             if (other) d_end = min(d_hi, (a_cur + __ffs(other) - 1) * npx - i0);   // last D row before that unit
@@ -578,7 +591,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
                 rf += (float)kRows;
                 // D rows d, d+1: D_y from registers, D_x from the neighbouring lanes.  A row past d_hi has D = 0
                 // exactly (or a weight from the rows of zeros); a row past d_end is the next segment's.
-                const bool two = !(kEdge || kTile) || d + 1 <= d_end;
+                const bool two = !(kEdge || kWhole) || d + 1 <= d_end;
 #pragma unroll
                 for (int k = 0; k < kRows; ++k) {
                     const float mid = k == 0 ? pmB : cur[k - 1];                         // phi[d+k]
@@ -643,9 +656,13 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
             int slot = 0, a_batch = a_cur;
             int rr = d + 1;   // phi row after the unit's first (counted from i0-1): rf is its re-based float
             for (int uu = 0; uu < nu; ++uu, rr += npx) {
-                if (uu != 0 && (uu & (kRebaseUnits - 1)) == 0) {
+                if (kTile && uu != 0 && (uu & (kRebaseUnits - 1)) == 0) {
                     rebase(rr, min(d_end + 1, rr + rebase_rows));
                     rf = 0.0f;
+                }
+                if (!kTile) {   // (a zonal CTA paces its column's zeros through this loop: about n/2 iterations' worth)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) zp.step();
                 }
                 const float rfu = rf - 1.0f;   // the unit's first row
                 const float fl = sample(rfu + (float)(npx - 1)), fn = sample(rfu + (float)npx);
@@ -694,7 +711,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
             int slot = 0, a_batch = a_cur;
             int rr = d + 1;   // next phi row to sample (counted from i0-1)
             for (int uu = 0; uu < nu; ++uu, rr += npx) {
-                if (uu != 0 && (uu & (kRebaseUnits - 1)) == 0) {
+                if (kTile && uu != 0 && (uu & (kRebaseUnits - 1)) == 0) {
                     rebase(rr, min(d_end + 1, rr + rebase_rows));
                     rf = 0.0f;
                 }
@@ -764,6 +781,7 @@ __device__ __forceinline__ void process_strip(const WfsDev &W, int i0, int i1, i
 // the inverse map, of the piece's open octagon: the box (qx0-1,qx1+1)x(qy0-1,qy1+1) cut by
 // sg0-2 < x+y < sg1+2 and dg0-2 < x-y < dg1+2.  So D(i,j) only for floor(jmin) <= j <= ceil(jmax) (one pixel
 // of stencil either side), clipped to the sensor.  Results go to shared memory for the other warps.
+template <bool kZPack>
 __device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, int qx0, int qx1, int qy0, int qy1, int sg0,
                                                    int sg1, int dg0, int dg1, int4 *s_box, int4 *s_win)
 {
@@ -808,6 +826,10 @@ __device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, 
                 }
             }
         }
+        if (kZPack && W.spb > 0 && r_i1 >= r_i0) {   // whole subaperture rows (the rows added hold phi = 0)
+            r_i0 = (r_i0 / W.n_pix) * W.n_pix;
+            r_i1 = min(W.M - 1, (r_i1 / W.n_pix + 1) * W.n_pix - 1);
+        }
         if (r_j1 >= r_j0 && r_i1 >= r_i0) {
             r_a0 = r_i0 / W.n_pix; r_b0 = r_j0 / W.n_pix;
             r_nb = r_j1 / W.n_pix - r_b0 + 1;
@@ -822,10 +844,10 @@ __device__ __forceinline__ void footprint_of_piece(const ImParams &p, int lane, 
 // All warps, after a barrier: fetch the IM rows of the windows' subapertures (needed only when the table
 // is stored: asynchronously, so that the store at the end waits for nothing), then sample the strips of
 // every sensor's footprint.
-template <bool kGtilt, bool kAligned, bool kRepair>
+template <bool kGtilt, bool kAligned, bool kRepair, bool kZPack>
 __device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, int lane, const int4 *s_box, const int4 *s_win,
                                                   int *s_next_ptr, const CellBox &cb, uint32_t tab_base, uint32_t krow_base,
-                                                  ZeroPacer &zp)
+                                                  ZeroPacer &zp, uint32_t scr)
 {
     // kAligned (every sensor of the launch has subapertures that fit a strip, spb > 0): strip t holds the spb
     // subaperture columns b0 + t*spb ... of the footprint's window; otherwise (giant subapertures) strips are
@@ -874,10 +896,10 @@ __device__ __forceinline__ void sample_footprints(const ImParams &p, int warp, i
         const uint32_t tab = tab_base + (uint32_t)W.tab_off * 4u;
         if (kAligned) {
             const int bA = b0 + (t - base) * spb;
-            process_strip<kGtilt, true, false, kRepair>(W, i0, i1, bA * W.n_pix, min(spb, b0 + nb - bA) * W.n_pix, cb, p.addr_bias, tab, a0, b0, nb, zp);
+            process_strip<kGtilt, true, kZPack ? 2 : 0, kRepair>(W, i0, i1, bA * W.n_pix, min(spb, b0 + nb - bA) * W.n_pix, cb, p.addr_bias, tab, a0, b0, nb, zp, scr);
         } else {
             const int jA = j0 + (t - base) * kStripCols;
-            process_strip<kGtilt, false, false, kRepair>(W, i0, i1, jA, min(kStripCols, j1 - jA + 1), cb, p.addr_bias, tab, a0, b0, nb, zp);
+            process_strip<kGtilt, false, 0, kRepair>(W, i0, i1, jA, min(kStripCols, j1 - jA + 1), cb, p.addr_bias, tab, a0, b0, nb, zp);
         }
     }
 }
@@ -910,8 +932,8 @@ __device__ __forceinline__ void scatter_table(const ImParams &p, const int4 *s_w
     }
 }
 
-template <bool kGtilt, bool kAligned, bool kRepair>
-__global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : SYNIM_STRIP_MINB) synim_strip_kernel(const __grid_constant__ ImParams p,
+template <bool kGtilt, bool kAligned, bool kRepair, bool kZPack>
+__global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : (kZPack ? 4 : SYNIM_STRIP_MINB)) synim_strip_kernel(const __grid_constant__ ImParams p,
                                                                                      const __grid_constant__ CUtensorMap tmap)
 {
     // [ TMA box: patch_pitch x patch_h floats | table: tab_floats | rows: tab_floats / 2 ints ]
@@ -926,6 +948,8 @@ __global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : SYNIM_STRIP_MINB)
     const uint32_t raw_base = smem_u32(patch);
     const uint32_t tab_base = raw_base + (uint32_t)(p.patch_pitch * p.patch_h) * 4u;
     const uint32_t krow_base = tab_base + (uint32_t)p.tab_floats * 4u;   // IM row of each (a, b) of the windows
+    // (kZPack) per-warp scratch of the packed edge-sum units, behind the rows
+    const uint32_t scr = kZPack ? krow_base + (uint32_t)(p.tab_floats >> 1) * 4u + (uint32_t)(warp * (kEdgeBatch * kEdgeSlotFloats)) * 4u : 0u;
 
     // dense modes (no bboxes): the support is the whole grid, split into pieces; blockIdx.y takes every
     // gridDim.y-th piece, and the pieces' slopes add up in the column, which the host has cleared
@@ -996,7 +1020,7 @@ __global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : SYNIM_STRIP_MINB)
             cb.s_lo = (float)(sg0 - 2 - (cb.x0 + cb.y0)) - 0.01f; cb.s_hi = (float)(sg1 + 2 - (cb.x0 + cb.y0)) + 0.01f;
             cb.d_lo = (float)(dg0 - 2 - (cb.x0 - cb.y0)) - 0.01f; cb.d_hi = (float)(dg1 + 2 - (cb.x0 - cb.y0)) + 0.01f;
             if (warp == 0 && lane < p.n_wfs)   // once per CTA, while the box is still in flight
-                footprint_of_piece(p, lane, qx0, qx1, qy0, qy1, sg0, sg1, dg0, dg1, s_box, s_win);
+                footprint_of_piece<kZPack>(p, lane, qx0, qx1, qy0, qy1, sg0, sg1, dg0, dg1, s_box, s_win);
             mbar_wait(&bar, parity);
             parity ^= 1u;
 
@@ -1009,7 +1033,7 @@ __global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : SYNIM_STRIP_MINB)
             }
             bar_sync(1, kComputeThreads);   // footprints (and a cleared ring) visible
 
-            sample_footprints<kGtilt, kAligned, kRepair>(p, warp, lane, s_box, s_win, &s_next, cb, tab_base, krow_base, zp);
+            sample_footprints<kGtilt, kAligned, kRepair, kZPack>(p, warp, lane, s_box, s_win, &s_next, cb, tab_base, krow_base, zp, scr);
             if (multi) {
                 cp_async_wait_all();
                 bar_sync(1, kComputeThreads);   // every warp is done with this box and this piece's table
@@ -1130,7 +1154,7 @@ __global__ void __launch_bounds__(kTileThreads, 2) synim_tile_kernel(const __gri
         if (it >= total) break;
         const int c = it / ns, sidx = it - c * ns;
         const int bA = b0 + sidx * spb, aA = a0 + c * cr, aE = min(aA + cr, a0 + na);
-        process_strip<kGtilt, true, true, kRepair>(W, aA * npx, aE * npx - 1, bA * npx, min(spb, b0 + nb - bA) * npx, cb, p.addr_bias,
+        process_strip<kGtilt, true, 1, kRepair>(W, aA * npx, aE * npx - 1, bA * npx, min(spb, b0 + nb - bA) * npx, cb, p.addr_bias,
                                           tab_base, a0, b0, nb, zp, scr);
     }
     __syncthreads();   // table complete
@@ -1158,15 +1182,19 @@ cudaError_t launch_strip(const ImParams &p, const void *tensor_map, size_t smem_
     for (int w = 0; w < p.n_wfs; ++w) aligned = aligned && p.wfs[w].spb > 0;
     for (int w = 0; w < p.n_wfs; ++w)
         if (!aligned && p.wfs[w].spb > 0) return cudaErrorInvalidValue;
-    auto kernel = repair ? (aligned ? synim_strip_kernel<false, true, true> : synim_strip_kernel<false, false, true>)
-                  : gtilt ? (aligned ? synim_strip_kernel<true, true, false> : synim_strip_kernel<true, false, false>)
-                          : (aligned ? synim_strip_kernel<false, true, false> : synim_strip_kernel<false, false, false>);
+    const bool zpack = p.unit_rows != 0 && aligned && !gtilt && !repair;
+    if (p.unit_rows != 0 && !zpack) return cudaErrorInvalidValue;   // (the host sets unit_rows only where it applies)
+    auto kernel = zpack ? synim_strip_kernel<false, true, false, true>
+                  : repair ? (aligned ? synim_strip_kernel<false, true, true, false> : synim_strip_kernel<false, false, true, false>)
+                  : gtilt ? (aligned ? synim_strip_kernel<true, true, false, false> : synim_strip_kernel<true, false, false, false>)
+                          : (aligned ? synim_strip_kernel<false, true, false, false> : synim_strip_kernel<false, false, false, false>);
+    if (zpack) smem_bytes += sizeof(float) * (size_t)(kComputeWarps * kEdgeBatch * kEdgeSlotFloats);
     // the opt-in shared-memory limit only ever has to grow (per device; a race sets it twice, harmlessly)
-    static size_t granted[6][64] = {};
+    static size_t granted[7][64] = {};
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    size_t &have = granted[(repair ? 4 : (gtilt ? 2 : 0)) + (aligned ? 1 : 0)][dev & 63];
+    size_t &have = granted[zpack ? 6 : (repair ? 4 : (gtilt ? 2 : 0)) + (aligned ? 1 : 0)][dev & 63];
     if (smem_bytes > have) {
         e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return e;

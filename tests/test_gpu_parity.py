@@ -616,3 +616,14 @@ def test_edge_repair_argument_errors(S):
     with pytest.raises(ValueError):
         S.interaction_matrix(geom, cube, None, S.affines_of(wl), repair_mask=mask, mode=S.SLOPES_GTILT)
     geom.destroy()
+
+
+def test_packed_zonal_walk_is_opt_in_and_agrees_with_the_oracle(S, monkeypatch):
+    """SYNIM_ZONAL_PACKED=1 (not the default until it has been timed): zonal footprints rounded out to whole units, their
+    edge-sum units sampled on the boundary rows and columns only.  Same matrix within the bar."""
+    monkeypatch.setenv("SYNIM_ZONAL_PACKED", "1")
+    for cfg, n in ((1, None), (3, 48), (2, 60), (4, 24)):
+        wl = W.make_config(cfg, max_modes=n)
+        assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
+    wl = W.make_config(1)
+    assert_parity(gpu_im(S, wl, hint=False, octagon=False, ld_pad=5), O.interaction_matrix(wl), wl)

@@ -409,6 +409,9 @@ def test_debug_build_traps_on_nothing(S, tmp_path):
             wl = W.make_config(cfg, max_modes=n)
             got = gpu_im(S, wl, **kw)
             assert np.isfinite(got).all()
+        wl = W.masked(W.make_config(1), W.make_pupil(80, 80.0, 0.14))          # edge repair, strips and tiles
+        for kw in ({}, dict(use_bbox=False)):
+            assert np.isfinite(gpu_im(S, wl, mask=wl.mask, **kw)).all()
     finally:
         S.LIB_PATH, S._lib = saved
 

@@ -1029,7 +1029,7 @@ __global__ void __launch_bounds__(kStripThreads, kRepair ? 4 : (kZPack ? 4 : SYN
             if (multi) {   // clear the ring just staged (pixels cw and ch are the far ring)
                 const uint32_t org = raw_base + (uint32_t)slack * 4u, rp4 = (uint32_t)p.patch_pitch * 4u;
                 for (int e = tid; e <= cb.cw; e += kComputeThreads) { sts_f32(org + (uint32_t)e * 4u, 0.0f); sts_f32(org + (uint32_t)cb.ch * rp4 + (uint32_t)e * 4u, 0.0f); }
-                for (int e = tid; e <= cb.ch; e += kComputeThreads) { sts_f32(org + (uint32_t)e * rp4, 0.0f); sts_f32(org + (uint32_t)e * rp4 + (uint32_t)cb.cw * 4u, 0.0f); }
+                for (int e = tid + 1; e < cb.ch; e += kComputeThreads) { sts_f32(org + (uint32_t)e * rp4, 0.0f); sts_f32(org + (uint32_t)e * rp4 + (uint32_t)cb.cw * 4u, 0.0f); }   // (the corners belong to the rows above)
             }
             bar_sync(1, kComputeThreads);   // footprints (and a cleared ring) visible
 

@@ -30,6 +30,16 @@ std::vector<WarpSync> warps;
 struct CtaSync { int arrived = 0; unsigned gen = 0; int acc = 0; int result[2] = {0, 0}; } cta;
 std::map<const char *, size_t> ranges;
 
+// Race tracking on the dynamic shared memory (a small racecheck): per 4-byte word the last writer and the last reader,
+// each with the CTA-barrier generation and the issuing warp's __syncwarp generation at the time.  Two accesses to a word,
+// at least one a plain write, conflict when they come from different warps with no CTA barrier in between, or from
+// different lanes of one warp with no __syncwarp in between (shuffles and votes converge the lanes but order no memory, so
+// they do not count).  Atomic adds conflict only with plain accesses.
+struct Access { int warp = -1, lane = 0; unsigned cta_gen = 0, warp_gen = 0; char kind = 0; };   // kind: 'w' plain, 'a' atomic, 'r' read
+std::vector<Access> last_write, last_read;
+std::vector<unsigned> syncwarp_gen;   // per warp
+unsigned long long races_found = 0;
+
 void trampoline() { (*cur_body)(); fibers[cur_fiber].done = true; ++progress; swapcontext(&fibers[cur_fiber].ctx, &sched_ctx); }
 int live_in_warp(int w)
 {
@@ -88,6 +98,9 @@ void launch(dim3 grid, dim3 block, size_t smemb, const std::function<void()> &bo
         smem = arena.data(); smem_bytes = smemb;
         fibers.assign(nt, Fiber());
         warps.assign((nt + 31) / 32, WarpSync());
+        last_write.assign(smemb / 4 + 1, Access());
+        last_read.assign(smemb / 4 + 1, Access());
+        syncwarp_gen.assign((nt + 31) / 32, 0u);
         cta = CtaSync();
         cur_body = &body;
         for (size_t t = 0; t < nt; ++t) {
@@ -128,8 +141,17 @@ void register_range(const void *p, size_t bytes)
 }
 void unregister_range(const void *p) { ranges.erase((const char *)p); }
 extern unsigned long long g_count_global;
+// (optional) one tracked buffer: how often each of its 4-byte words is stored with __stcs -- the tile kernel's claim that
+// every slope is stored exactly once is checked with this
+static const char *track_base = nullptr;
+static std::vector<unsigned char> track_count;
 void check_global(const void *p, size_t bytes, const char *what)
 {
+    if (track_base && what[0] == '_' && what[2] == 's') {   // "__stcs"
+        const char *c = (const char *)p;
+        if (c >= track_base && c + bytes <= track_base + track_count.size() * 4)
+            for (size_t k = 0; k < bytes / 4; ++k) { unsigned char &n = track_count[(c - track_base) / 4 + k]; if (n < 255) ++n; }
+    }
     ++g_count_global;
     const char *c = (const char *)p;
     auto it = ranges.upper_bound(c);
@@ -137,6 +159,13 @@ void check_global(const void *p, size_t bytes, const char *what)
     fail("%s: global access of %zu bytes at %p is outside every registered buffer", what, bytes, p);
 }
 unsigned long long g_count_shared_ld = 0, g_count_shared_st = 0, g_count_gather = 0, g_count_global = 0;
+void note_syncwarp() { if (cur_fiber >= 0 && (cur_fiber & 31) == 0) ++syncwarp_gen[cur_fiber >> 5]; }
+static void conflict(const char *what, const char *how, uint32_t addr, const Access &o)
+{
+    ++races_found;
+    fail("%s: shared-memory race (%s) on window offset %u: the other access came from warp %d lane %d with no %s in between", what, how,
+         addr - kSmemBase, o.warp, o.lane, o.warp == (cur_fiber >> 5) ? "__syncwarp" : "CTA barrier");
+}
 char *shared_ptr(uint32_t addr, size_t bytes, const char *what)
 {
     if (what[0] == 'l') ++g_count_shared_ld; else ++g_count_shared_st;
@@ -144,6 +173,26 @@ char *shared_ptr(uint32_t addr, size_t bytes, const char *what)
         fail("%s: shared access of %zu bytes at window offset %lld is outside the CTA's %zu bytes of dynamic shared memory", what, bytes,
              (long long)addr - (long long)kSmemBase, smem_bytes);
     if (addr % bytes) fail("%s: misaligned shared access", what);
+    if (cur_fiber >= 0 && what[0] != 't') {   // (TMA writes are ordered by their mbarrier; its waits are not modelled)
+        const int w = cur_fiber >> 5, l = cur_fiber & 31;
+        const char kind = what[0] == 'l' ? 'r' : (what[0] == 'r' ? 'a' : 'w');
+        const size_t word = (addr - kSmemBase) / 4;
+        const unsigned wg = syncwarp_gen[w];
+        auto clashes = [&](const Access &o) {
+            if (o.warp < 0) return false;
+            if (o.warp != w) return o.cta_gen == cta.gen;
+            return o.lane != l && o.warp_gen == wg && o.cta_gen == cta.gen;
+        };
+        Access &lw = last_write[word], &lr = last_read[word];
+        if (kind == 'r') {
+            if (clashes(lw)) conflict(what, "read after write", addr, lw);
+            lr.warp = w; lr.lane = l; lr.cta_gen = cta.gen; lr.warp_gen = wg; lr.kind = 'r';
+        } else {
+            if (clashes(lw) && !(kind == 'a' && lw.kind == 'a')) conflict(what, "write after write", addr, lw);
+            if (clashes(lr)) conflict(what, "write after read", addr, lr);
+            lw.warp = w; lw.lane = l; lw.cta_gen = cta.gen; lw.warp_gen = wg; lw.kind = kind;
+        }
+    }
     return smem + (addr - kSmemBase);
 }
 uint32_t shared_addr(const void *p)
@@ -182,5 +231,7 @@ cudaError_t cudaGetDriverEntryPoint(const char *, void **fn, int, cudaDriverEntr
 }
 
 extern "C" void emu_counters(unsigned long long *out) { out[0] = emu::g_count_shared_ld; out[1] = emu::g_count_shared_st; out[2] = emu::g_count_gather; out[3] = emu::g_count_global; emu::g_count_shared_ld = emu::g_count_shared_st = emu::g_count_gather = emu::g_count_global = 0; }
+extern "C" void emu_track_stores(const void *p, size_t bytes) { emu::track_base = (const char *)p; emu::track_count.assign(bytes / 4, 0); }
+extern "C" void emu_store_counts(unsigned char *out) { memcpy(out, emu::track_count.data(), emu::track_count.size()); emu::track_base = nullptr; }
 extern "C" void emu_register(const void *p, size_t n) { emu::register_range(p, n); }
 extern "C" void emu_unregister(const void *p) { emu::unregister_range(p); }

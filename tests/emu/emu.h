@@ -36,6 +36,7 @@ int cta_barrier_or(int pred);
 // warp collective: every live lane contributes 8 bytes; afterwards all 32 slots are readable until the next collective
 const uint64_t *warp_gather(uint64_t mine);
 int lane_id();
+void note_syncwarp();   // (race tracking: a __syncwarp orders the warp's shared-memory accesses)
 void register_range(const void *p, size_t bytes);
 void unregister_range(const void *p);
 void check_global(const void *p, size_t bytes, const char *what);
@@ -81,7 +82,7 @@ static inline unsigned __ballot_sync(unsigned, int pred)
     unsigned m = 0; for (int l = 0; l < 32; ++l) if (all[l] & 1u) m |= 1u << l;
     return m;
 }
-static inline void __syncwarp(unsigned = 0xffffffffu) { emu::warp_gather(0); }
+static inline void __syncwarp(unsigned = 0xffffffffu) { emu::warp_gather(0); emu::note_syncwarp(); emu::warp_gather(0); }
 static inline void __syncthreads() { emu::cta_barrier(); }
 static inline int __syncthreads_or(int p) { return emu::cta_barrier_or(p); }
 template <typename T> static inline T __ldg(const T *p) { emu::check_global(p, sizeof(T), "__ldg"); return *p; }

@@ -64,7 +64,10 @@ class Emu:
         L.synim_destroy.restype = None
         L.synim_last_error.restype = ctypes.c_char_p
         L.emu_register.argtypes = [vp, ctypes.c_size_t]
+        L.emu_track_stores.argtypes = [vp, ctypes.c_size_t]
+        L.emu_store_counts.argtypes = [vp]
         self.L = L
+        self.store_counts = None     # after interaction_matrix(count_stores=True): uint8 [n_modes][rows + ld_pad]
 
     def reg(self, a: np.ndarray) -> np.ndarray:
         self.L.emu_register(a.ctypes.data, a.nbytes)
@@ -102,7 +105,7 @@ class Emu:
         return h, keep
 
     def interaction_matrix(self, wl, use_bbox=True, ld_pad=0, hint=True, octagon=True, mode=0, affines=None, scales=None,
-                           mask=None, threshold=0.999999):
+                           mask=None, threshold=0.999999, count_stores=False):
         """The IM of a workload through the emulated C ABI -> float64 [rows][n_modes] (as tests/test_gpu_parity.gpu_im)."""
         L = self.L
         h, keep = self.geometry(wl.wfs, wl.ny, wl.nx)
@@ -130,6 +133,8 @@ class Emu:
         if scales is None:
             scales = [w.slope_scale for w in wl.wfs]
         arr = S._affine_array(affines, scales)
+        if count_stores:
+            L.emu_track_stores(out.ctypes.data, out.nbytes)
         if mask is not None:
             mk = self.reg(np.ascontiguousarray(mask, dtype=np.float32).copy())
             self.chk(L.synim_interaction_matrix_repaired(h, cube.ctypes.data, wl.n_modes, bptr, dptr, bw, bh, arr, mk.ctypes.data,
@@ -137,6 +142,10 @@ class Emu:
         else:
             self.chk(L.synim_interaction_matrix(h, cube.ctypes.data, wl.n_modes, bptr, dptr, bw, bh, arr, mode, out.ctypes.data,
                                                 rows + ld_pad, None))
+        if count_stores:
+            cnt = np.zeros(out.shape, np.uint8)
+            L.emu_store_counts(cnt.ctypes.data)
+            self.store_counts = cnt
         L.synim_destroy(h)
         if ld_pad:
             assert np.isnan(out[:, rows:]).all()          # padding rows are left untouched

@@ -57,10 +57,18 @@ def check(got, ref, wl, tol=TOL):
     return worst
 
 
+def emu_last_nonzero(emu, wl):
+    """Where the strip kernel's slope table held a non-zero value (it stores only those on top of the zeros): the
+    non-zero entries of the matrix itself."""
+    return emu.interaction_matrix(wl).T != 0
+
+
 def test_strip_kernel_zonal_modes(emu):
     wl = W.make_config(1, max_modes=30)
     ref = O.interaction_matrix(wl)
-    check(emu.interaction_matrix(wl), ref, wl)
+    check(emu.interaction_matrix(wl, count_stores=True), ref, wl)
+    cnt = emu.store_counts                             # the column's zeros once, the non-zero slopes once more on top
+    assert cnt.min() == 1 and cnt.max() == 2 and ((cnt == 2) == (emu_last_nonzero(emu, wl))).all()
     check(emu.interaction_matrix(wl, hint=False, octagon=False, ld_pad=3), ref, wl)
     check(emu.interaction_matrix(wl, mode=1), O.interaction_matrix(wl, mode=O.GTILT), wl)
     for cfg, n in ((3, 6), (4, 4)):                    # six rotated LGS sensors; the cone effect and giant NGS subapertures
@@ -75,7 +83,8 @@ def test_tile_kernel_dense_modes(emu):
     check(emu.interaction_matrix(wl, use_bbox=False, ld_pad=5), O.interaction_matrix(wl), wl)
     check(emu.interaction_matrix(wl, use_bbox=False, mode=1), O.interaction_matrix(wl, mode=O.GTILT), wl)
     wl = W.make_config(5, max_modes=1)
-    assert check(emu.interaction_matrix(wl), O.interaction_matrix(wl), wl) < 3e-6
+    assert check(emu.interaction_matrix(wl, count_stores=True), O.interaction_matrix(wl), wl) < 3e-6
+    assert (emu.store_counts == 1).all()               # output-stationary: every slope is stored exactly once
 
 
 def test_edge_repair_in_both_kernels(emu):

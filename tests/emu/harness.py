@@ -68,6 +68,7 @@ class Emu:
         L.emu_store_counts.argtypes = [vp]
         self.L = L
         self.store_counts = None     # after interaction_matrix(count_stores=True): uint8 [n_modes][rows + ld_pad]
+        self.pre_launch = None       # optional callable run right before the interaction-matrix call (op_counts.py)
 
     def reg(self, a: np.ndarray) -> np.ndarray:
         self.L.emu_register(a.ctypes.data, a.nbytes)
@@ -133,6 +134,8 @@ class Emu:
         if scales is None:
             scales = [w.slope_scale for w in wl.wfs]
         arr = S._affine_array(affines, scales)
+        if self.pre_launch:
+            self.pre_launch()
         if count_stores:
             L.emu_track_stores(out.ctypes.data, out.nbytes)
         if mask is not None:

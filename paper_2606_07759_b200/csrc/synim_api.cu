@@ -86,6 +86,11 @@ struct synim_geometry {
         char *h_stage[2] = {nullptr, nullptr}; size_t h_stage_bytes[2] = {0, 0};
     };
     mutable Pipe pipe;
+    // the last tile plan of every sensor (dense modes): planning simulates bank conflicts (about a millisecond of host
+    // time per sensor), and an on-line loop calls with the same transforms again and again
+    struct PlanMemo { bool set = false; double key[7] = {0, 0, 0, 0, 0, 0, 0}; int ns = 0, nr = 0, pitch = 0, h = 0; bool fits = false; };
+    mutable std::mutex plan_lock;
+    mutable std::vector<PlanMemo> plans;
 };
 
 namespace {
@@ -608,8 +613,22 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
             bool fits = true;
             int tiles = 0, box_floats = 0, tab = 0;
             for (int w = 0; w < nw && fits; ++w) {
-                TilePlan tp;
-                fits = plan_tiles(p.wfs[w], budget / sizeof(float), reach, &tp);
+                TilePlan tp = {0, 0, 0, 0};
+                {
+                    std::lock_guard<std::mutex> memo_guard(g->plan_lock);
+                    if (g->plans.size() != g->wfs.size()) g->plans.assign(g->wfs.size(), synim_geometry::PlanMemo());
+                    synim_geometry::PlanMemo &pm = g->plans[w0 + w];
+                    const synim::WfsDev &dd = p.wfs[w];
+                    const double key[7] = {dd.fwd[0], dd.fwd[1], dd.fwd[2], dd.fwd[3], dd.fwd[4], dd.fwd[5], (double)reach};
+                    if (!pm.set || std::memcmp(pm.key, key, sizeof(key)) != 0) {
+                        pm.fits = plan_tiles(dd, budget / sizeof(float), reach, &tp);
+                        pm.ns = tp.ns; pm.nr = tp.nr; pm.pitch = tp.pitch; pm.h = tp.h;
+                        std::memcpy(pm.key, key, sizeof(key));
+                        pm.set = true;
+                    }
+                    fits = pm.fits;
+                    tp.ns = pm.ns; tp.nr = pm.nr; tp.pitch = pm.pitch; tp.h = pm.h;
+                }
                 if (!fits) break;
                 synim::WfsDev &d = p.wfs[w];
                 d.tile_ns = tp.ns; d.tile_nr = tp.nr; d.box_pitch = tp.pitch; d.box_h = tp.h;

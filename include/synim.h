@@ -43,7 +43,7 @@ extern "C" {
 #endif
 
 #define SYNIM_VERSION_MAJOR 0
-#define SYNIM_VERSION_MINOR 1
+#define SYNIM_VERSION_MINOR 2
 
 typedef struct synim_geometry synim_geometry; /* opaque, library-owned */
 

@@ -207,3 +207,64 @@ print("ok %.2e" % err)
     res = subprocess.run([sys.executable, "-c", code, root, os.path.join(HERE, "emu"), os.path.join(emu.dir, "libsynim_emu.so")],
                          capture_output=True, text=True, env=env, timeout=600, cwd=root)
     assert res.returncode == 0 and res.stdout.startswith("ok"), res.stderr[-2000:]
+
+
+def _shard_worker(rank, world, port, lib_path, q):
+    """One rank of a two-process gloo job: its sharding.partition_modes range of config 1 through the EMULATED library,
+    then sharding.sharded_columns' all_gather of the column blocks."""
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, os.path.join(HERE, "emu"))
+    import harness
+    from paper_2606_07759_b200 import sharding
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        e = harness.Emu(lib_path)
+        wl = W.make_config(1, max_modes=21)
+
+        def compute(b, e_):
+            import copy
+            part = copy.copy(wl)
+            part.cube = np.ascontiguousarray(wl.cube[b:e_])
+            part.bbox = np.ascontiguousarray(wl.bbox[b:e_])
+            if e_ == b:
+                return torch.zeros((0, wl.n_rows), dtype=torch.float32)
+            return torch.from_numpy(e.interaction_matrix(part).T.astype(np.float32).copy())
+        full, (b, e_) = sharding.sharded_columns(wl.n_modes, compute, gather=True)
+        q.put((rank, b, e_, full.numpy()))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+def test_two_gloo_ranks_shard_the_modes_through_the_kernels(emu):
+    """SURVEY sec. 8(e) on CPU with the kernels in the loop (the stand-in `compute` of tests/test_sharding_gloo.py replaced
+    by the emulated library): two ranks, contiguous mode ranges, no exchange but the final all_gather; the gathered matrix
+    is bit for bit the unsharded one."""
+    import socket
+    import torch.multiprocessing as mp
+    from paper_2606_07759_b200 import sharding
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    lib = os.path.join(emu.dir, "libsynim_emu.so")
+    procs = [ctx.Process(target=_shard_worker, args=(r, world, port, lib, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = [q.get(timeout=240) for _ in range(world)]
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    wl = W.make_config(1, max_modes=21)
+    whole = emu.interaction_matrix(wl).T.astype(np.float32)
+    ranges = sharding.partition_modes(wl.n_modes, world)
+    for rank, b, e_, full in got:
+        assert (b, e_) == ranges[rank]
+        assert np.array_equal(full, whole)
+    check(whole.T.astype(np.float64), O.interaction_matrix(wl), wl)

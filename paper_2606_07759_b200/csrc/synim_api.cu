@@ -377,7 +377,10 @@ static bool plan_tiles(const synim::WfsDev &d, size_t budget_floats, int reach, 
         box(ns, nr, &pitch, &h);
         if (pitch <= 256 && h <= 256 && (size_t)pitch * h + 3 * (size_t)ns * d.spb * nr <= budget_floats) break;
         if (ns == 1 && nr == 1) return false;
-        if (nr > 1 && (nr * d.n_pix >= ns * strip_px || ns == 1)) --nr; else --ns;
+        // shrink the height first while the tile is not much flatter than wide: a CTA has one warp per strip, so a tile
+        // of fewer strips than warps leaves warps idle, whereas fewer rows only shorten the strips
+        const bool keep_width = ns <= synim::kTileWarpsPerCta && 10 * nr * d.n_pix >= 6 * ns * strip_px;
+        if (nr > 1 && (keep_width || nr * d.n_pix >= ns * strip_px || ns == 1)) --nr; else --ns;
     }
     auto even_out = [&](int *pns, int *pnr) {
         const int ty = (d.n_subap + *pnr - 1) / *pnr, tx = (n_strips + *pns - 1) / *pns;

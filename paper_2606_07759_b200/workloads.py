@@ -362,7 +362,7 @@ def make_dictionary(n_layers: int = 12, acts_across: int = 66, max_modes: Option
     between 0 and 22 km, six LGS WFS of 68x68 subapertures, meta-pupil grids of 480^2 ... 690^2 pixels): one
     Workload per component, all looking through the SAME six sensors (the config-3 sensors, 45 arcsec off axis on a
     hexagonal ring, 90 km range), each with its own grid, cone factor and footprints (the physical records carry
-    dm_height_m).  Zonal Gaussian influence functions on a centred grid of ``acts_across`` actuators across the
+    dm_height_m); every third layer is seen anamorphically and every fourth with a sub-pixel alignment scale s != 1.  Zonal Gaussian influence functions on a centred grid of ``acts_across`` actuators across the
     meta-pupil; ``max_modes`` keeps a seeded subset per layer.  Stand-in for the MORFEO modal bases, which are not
     available here."""
     npix, nsub = 7, 68
@@ -385,6 +385,10 @@ def make_dictionary(n_layers: int = 12, acts_across: int = 66, max_modes: Option
             q = dict(p)
             q.update(dm_height_m=1000.0 * h_km, gs_range_m=90000.0, gs_theta_arcsec=45.0, gs_azimuth_deg=60.0 * k,
                      src_pixel_pitch_m=pitch_m)
+            if li % 3 == 1:          # an anamorphic sensor-to-layer registration ("anamorphic distortions")
+                q.update(mag_x=q["mag_x"] * 1.012, mag_y=q["mag_y"] * 0.991)
+            if li % 4 == 2:          # a sub-pixel alignment scale s != 1 (reading R11)
+                q.update(wfs_pitch_src_px=1.003)
             wfs.append(WfsInput(nsub, npix, pup, val, q))
         out.append(Workload(f"dictionary layer {li} ({h_km:.1f} km, {n}x{n})", 0, n, n, cube, bbox, wfs, keep))
     return out

@@ -85,6 +85,13 @@ def test_tile_kernel_dense_modes(emu):
     wl = W.make_config(5, max_modes=1)
     assert check(emu.interaction_matrix(wl, count_stores=True), O.interaction_matrix(wl), wl) < 3e-6
     assert (emu.store_counts == 1).all()               # output-stationary: every slope is stored exactly once
+    # a sensor demagnified until no tile fits a TMA box (falls back to source-space pieces), and a strongly magnified one
+    cube = W.random_smooth_cube(2, 64, 64, 3)
+    pup = W.make_pupil(42, 42.0, 0.0)
+    for mag in (0.05, 3.0):
+        s = [W.WfsInput(6, 7, pup, W.valid_subaps(pup, 6, 7), W.physical(mag_x=mag, mag_y=mag, rot_deg=20.0))]
+        wl = W.Workload(f"mag {mag}", 0, 64, 64, cube, None, s)
+        check(emu.interaction_matrix(wl), O.interaction_matrix(wl), wl)
 
 
 def test_edge_repair_in_both_kernels(emu):

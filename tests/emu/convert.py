@@ -12,13 +12,13 @@ import shutil
 SRC = os.path.join(os.path.dirname(os.path.abspath(__file__)), "..", "..", "paper_2606_07759_b200", "csrc")
 
 BODIES = {
-    "mbar_init": "{ (void)bar; (void)count; }",
+    "mbar_init": "{ emu::mbar_init(bar, count); }",
     "fence_barrier_init": "{ }",
     "fence_proxy_async": "{ }",
-    "mbar_expect_tx": "{ (void)bar; (void)bytes; }",
-    "mbar_try_wait": "{ (void)bar; (void)parity; return true; }",
-    "tma_load_box": "{ (void)bar; emu_tma(dst, map, x, y, z); }",
-    "tma_load_box_plain": "{ (void)bar; emu_tma(dst, map, x, y, z); }",
+    "mbar_expect_tx": "{ emu::mbar_arrive_expect_tx(bar, bytes); }",
+    "mbar_try_wait": "{ return emu::mbar_try_wait(bar, parity); }",
+    "tma_load_box": "{ emu::mbar_complete_tx(bar, emu_tma(dst, map, x, y, z)); }",
+    "tma_load_box_plain": "{ emu::mbar_complete_tx(bar, emu_tma(dst, map, x, y, z)); }",
     "lds_f32": '{ return *(float *)emu::shared_ptr(addr, 4, "lds_f32"); }',
     "lds_s32": '{ return *(int *)emu::shared_ptr(addr, 4, "lds_s32"); }',
     "sts_f32": '{ *(float *)emu::shared_ptr(addr, 4, "sts_f32") = v; }',
@@ -30,7 +30,7 @@ BODIES = {
     "wld": '{ emu::check_global(p, 4, "wld"); return *p; }',
 }
 TMA = r'''
-static inline void emu_tma(void *dst, const void *map, int x, int y, int z)
+static inline uint32_t emu_tma(void *dst, const void *map, int x, int y, int z)   // -> bytes delivered
 {
     EmuTensorMap m; memcpy(&m, map, sizeof(m));
     const uint32_t a = emu::shared_addr(dst);
@@ -49,6 +49,7 @@ static inline void emu_tma(void *dst, const void *map, int x, int y, int z)
             }
             d[r * m.box[0] + c] = v;
         }
+    return m.box[0] * m.box[1] * m.box[2] * 4u;
 }
 '''
 

@@ -87,10 +87,72 @@ static int cta_sync(int pred)
 void cta_barrier() { cta_sync(0); }
 int cta_barrier_or(int pred) { return cta_sync(pred != 0); }
 
-void launch(dim3 grid, dim3 block, size_t smemb, const std::function<void()> &body)
+// ---- launch rules the hardware enforces: opt-in dynamic shared memory, grid limits ----------------------------------
+static std::map<const void *, int> max_dyn_smem;
+constexpr int kOptInSmem = 232448, kDefaultSmem = 48 << 10;
+int set_max_dynamic_smem(const void *fn, int bytes)
+{
+    if (bytes < 0 || bytes > kOptInSmem) return 1;   // cudaErrorInvalidValue
+    max_dyn_smem[fn] = bytes;
+    return 0;
+}
+
+// ---- mbarrier: the current phase completes when its pending arrivals and its transaction bytes are both zero --------
+namespace {
+struct MBar { bool init = false; int count = 0, pending = 0; long long tx = 0; unsigned phase = 0; };
+std::map<const void *, MBar> mbars;
+MBar &mbar_of(const void *bar, const char *what)
+{
+    auto it = mbars.find(bar);
+    if (it == mbars.end() || !it->second.init) fail("%s on an mbarrier this CTA has not initialised", what);
+    return it->second;
+}
+void mbar_settle(MBar &b) { if (b.pending == 0 && b.tx == 0) { ++b.phase; b.pending = b.count; ++progress; } }
+}  // namespace
+void mbar_init(const void *bar, int count)
+{
+    if (count < 1) fail("mbarrier.init with count %d", count);
+    MBar &b = mbars[bar];
+    b = MBar(); b.init = true; b.count = b.pending = count;
+}
+void mbar_arrive_expect_tx(const void *bar, uint32_t bytes)
+{
+    MBar &b = mbar_of(bar, "mbarrier.arrive.expect_tx");
+    if (b.pending <= 0) fail("mbarrier.arrive beyond the barrier's arrival count");
+    if (bytes >= (1u << 20)) fail("mbarrier.expect_tx of %u bytes: the transaction count holds less than 2^20", bytes);
+    b.tx += bytes; --b.pending;
+    mbar_settle(b);
+}
+void mbar_complete_tx(const void *bar, uint32_t bytes)
+{
+    MBar &b = mbar_of(bar, "TMA complete_tx");
+    b.tx -= bytes;
+    mbar_settle(b);
+}
+bool mbar_try_wait(const void *bar, uint32_t parity)
+{
+    MBar &b = mbar_of(bar, "mbarrier.try_wait");
+    if (parity > 1) fail("mbarrier.try_wait.parity with parity %u", parity);
+    if ((b.phase & 1u) != parity) {
+        if (b.phase == 0) fail("mbarrier.try_wait on the parity of a phase that never ran (returns at once on hardware: a race)");
+        return true;
+    }
+    yield();   // the phase with this parity is still open: somebody else has to complete it
+    return false;
+}
+
+void launch(const void *fn, dim3 grid, dim3 block, size_t smemb, const std::function<void()> &body)
 {
     const size_t nt = (size_t)block.x * block.y * block.z;
     if (nt == 0 || nt > 1024) fail("bad block size");
+    if (grid.x == 0 || grid.y == 0 || grid.z == 0 || grid.x > 2147483647u || grid.y > 65535u || grid.z > 65535u)
+        fail("bad grid (%u, %u, %u): the launch fails on hardware", grid.x, grid.y, grid.z);
+    {
+        auto it = max_dyn_smem.find(fn);
+        const size_t granted = it == max_dyn_smem.end() ? (size_t)kDefaultSmem : std::max<size_t>((size_t)it->second, (size_t)kDefaultSmem);
+        if (smemb > granted)
+            fail("launch with %zu bytes of dynamic shared memory, but this kernel was granted %zu (cudaFuncSetAttribute on THIS instantiation)", smemb, granted);
+    }
     while (stack_pool.size() < nt) stack_pool.push_back((char *)malloc(kStack));
     std::vector<char> arena(smemb + 64, 0);
     for (unsigned bz = 0; bz < grid.z; ++bz) for (unsigned by = 0; by < grid.y; ++by) for (unsigned bx = 0; bx < grid.x; ++bx) {
@@ -102,6 +164,7 @@ void launch(dim3 grid, dim3 block, size_t smemb, const std::function<void()> &bo
         last_read.assign(smemb / 4 + 1, Access());
         syncwarp_gen.assign((nt + 31) / 32, 0u);
         cta = CtaSync();
+        mbars.clear();   // static __shared__ barriers are garbage until this CTA initialises them
         cur_body = &body;
         for (size_t t = 0; t < nt; ++t) {
             Fiber &f = fibers[t];
@@ -153,6 +216,11 @@ void check_global(const void *p, size_t bytes, const char *what)
             for (size_t k = 0; k < bytes / 4; ++k) { unsigned char &n = track_count[(c - track_base) / 4 + k]; if (n < 255) ++n; }
     }
     ++g_count_global;
+    if (bytes <= 16 && ((uintptr_t)p % bytes) != 0) fail("%s: misaligned global access of %zu bytes at %p", what, bytes, p);
+    check_range(p, bytes, what);
+}
+void check_range(const void *p, size_t bytes, const char *what)
+{
     const char *c = (const char *)p;
     auto it = ranges.upper_bound(c);
     if (it != ranges.begin()) { --it; if (c >= it->first && c + bytes <= it->first + it->second) return; }

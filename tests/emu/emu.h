@@ -13,7 +13,7 @@
 
 struct dim3 { unsigned x, y, z; dim3(unsigned a = 1, unsigned b = 1, unsigned c = 1) : x(a), y(b), z(c) {} };
 struct uint3 { unsigned x, y, z; };
-struct float4 { float x, y, z, w; };
+struct alignas(16) float4 { float x, y, z, w; };
 struct alignas(16) int4 { int x, y, z, w; };
 struct alignas(8) int2 { int x, y; };
 static inline float4 make_float4(float a, float b, float c, float d) { return float4{a, b, c, d}; }
@@ -30,7 +30,13 @@ extern size_t smem_bytes;
 constexpr uint32_t kSmemBase = 4096;   // shared-window address of arena byte 0 (small negative offsets stay detectable)
 void yield();
 void fail(const char *fmt, ...);
-void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &body);
+void launch(const void *fn, dim3 grid, dim3 block, size_t smem, const std::function<void()> &body);
+int set_max_dynamic_smem(const void *fn, int bytes);   // cudaFuncSetAttribute(MaxDynamicSharedMemorySize)
+// mbarrier model (one CTA runs at a time; TMA is synchronous): arrival count, transaction bytes, phase parity
+void mbar_init(const void *bar, int count);
+void mbar_arrive_expect_tx(const void *bar, uint32_t bytes);
+void mbar_complete_tx(const void *bar, uint32_t bytes);
+bool mbar_try_wait(const void *bar, uint32_t parity);
 void cta_barrier();
 int cta_barrier_or(int pred);
 // warp collective: every live lane contributes 8 bytes; afterwards all 32 slots are readable until the next collective
@@ -39,7 +45,8 @@ int lane_id();
 void note_syncwarp();   // (race tracking: a __syncwarp orders the warp's shared-memory accesses)
 void register_range(const void *p, size_t bytes);
 void unregister_range(const void *p);
-void check_global(const void *p, size_t bytes, const char *what);
+void check_global(const void *p, size_t bytes, const char *what);   // one access: in range and naturally aligned
+void check_range(const void *p, size_t bytes, const char *what);    // a byte range (memset, memcpy)
 char *shared_ptr(uint32_t addr, size_t bytes, const char *what);
 uint32_t shared_addr(const void *p);
 }
@@ -109,7 +116,7 @@ static inline void __trap() { emu::fail("__trap()"); }
 using std::min; using std::max;
 static inline int min(int a, unsigned b) { return std::min(a, (int)b); }
 
-#define EMU_LAUNCH(kernel, grid, block, smemb, ...) emu::launch(dim3(grid), dim3(block), (size_t)(smemb), [&]() { kernel(__VA_ARGS__); })
+#define EMU_LAUNCH(kernel, grid, block, smemb, ...) emu::launch((const void *)(kernel), dim3(grid), dim3(block), (size_t)(smemb), [&]() { kernel(__VA_ARGS__); })
 
 // ---- runtime API shim -------------------------------------------------------------------------------------------
 typedef int cudaError_t;
@@ -124,7 +131,10 @@ static inline const char *cudaGetErrorString(cudaError_t e) { return e == 0 ? "n
 static inline cudaError_t cudaGetLastError() { return cudaSuccess; }
 static inline cudaError_t cudaGetDevice(int *d) { *d = 0; return cudaSuccess; }
 static inline cudaError_t cudaDeviceGetAttribute(int *v, int attr, int) { *v = attr == cudaDevAttrComputeCapabilityMajor ? 10 : 232448; return cudaSuccess; }
-template <typename F> static inline cudaError_t cudaFuncSetAttribute(F, int, int) { return cudaSuccess; }
+template <typename F> static inline cudaError_t cudaFuncSetAttribute(F f, int attr, int v)
+{
+    return attr == cudaFuncAttributeMaxDynamicSharedMemorySize ? emu::set_max_dynamic_smem((const void *)f, v) : cudaSuccess;
+}
 cudaError_t cudaMalloc(void **p, size_t n);
 cudaError_t cudaFree(void *p);
 static inline cudaError_t cudaMallocAsync(void **p, size_t n, cudaStream_t) { return cudaMalloc(p, n); }
@@ -132,10 +142,10 @@ static inline cudaError_t cudaFreeAsync(void *p, cudaStream_t) { return cudaFree
 static inline cudaError_t cudaMallocHost(void **p, size_t n) { *p = malloc(n); return *p ? cudaSuccess : cudaErrorMemoryAllocation; }
 static inline cudaError_t cudaFreeHost(void *p) { free(p); return cudaSuccess; }
 static inline cudaError_t cudaMemcpyAsync(void *d, const void *s, size_t n, cudaMemcpyKind, cudaStream_t) { memcpy(d, s, n); return cudaSuccess; }
-static inline cudaError_t cudaMemsetAsync(void *d, int v, size_t n, cudaStream_t) { emu::check_global(d, n, "cudaMemsetAsync"); memset(d, v, n); return cudaSuccess; }
+static inline cudaError_t cudaMemsetAsync(void *d, int v, size_t n, cudaStream_t) { emu::check_range(d, n, "cudaMemsetAsync"); memset(d, v, n); return cudaSuccess; }
 static inline cudaError_t cudaMemset2DAsync(void *d, size_t pitch, int v, size_t w, size_t h, cudaStream_t)
 {
-    for (size_t r = 0; r < h; ++r) { emu::check_global((char *)d + r * pitch, w, "cudaMemset2DAsync"); memset((char *)d + r * pitch, v, w); }
+    for (size_t r = 0; r < h; ++r) { emu::check_range((char *)d + r * pitch, w, "cudaMemset2DAsync"); memset((char *)d + r * pitch, v, w); }
     return cudaSuccess;
 }
 static inline cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSuccess; }

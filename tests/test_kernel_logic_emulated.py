@@ -74,6 +74,13 @@ def test_strip_kernel_zonal_modes(emu):
     for cfg, n in ((3, 6), (4, 4)):                    # six rotated LGS sensors; the cone effect and giant NGS subapertures
         wl = W.make_config(cfg, max_modes=n)
         check(emu.interaction_matrix(wl), O.interaction_matrix(wl), wl)
+    # supports larger than the staged box and no size hint: one CTA walks nine pieces, re-arming its mbarrier for each
+    # (the emulated barrier checks the transaction bytes and the phase parity of every wait)
+    cube = W.random_smooth_cube(2, 160, 160, 3)
+    pup = W.make_pupil(60, 60.0, 0.0)
+    s = [W.WfsInput(10, 6, pup, W.valid_subaps(pup, 10, 6), W.physical(rot_deg=10.0, mag_x=0.4, mag_y=0.4))]
+    wl = W.Workload("split supports", 0, 160, 160, cube, W.tight_bboxes(cube), s)
+    check(emu.interaction_matrix(wl, hint=False), O.interaction_matrix(wl), wl)
 
 
 def test_tile_kernel_dense_modes(emu):

@@ -273,8 +273,7 @@ uint32_t shared_addr(const void *p)
 
 cudaError_t cudaMalloc(void **p, size_t n)
 {
-    *p = aligned_alloc(256, (n + 255) & ~(size_t)255);
-    if (!*p) return cudaErrorMemoryAllocation;
+    if (posix_memalign(p, 256, n ? n : 1) != 0) { *p = nullptr; return cudaErrorMemoryAllocation; }   // (exactly n bytes: a sanitizer sees the end)
     memset(*p, 0xA5, n);   // device memory starts as garbage
     emu::register_range(*p, n);
     return cudaSuccess;

@@ -29,7 +29,9 @@ def build(out_dir: str, defines=()) -> str:
     gen = os.path.join(out_dir, "gen")
     srcs = convert.convert_all(gen)
     lib = os.path.join(out_dir, "libsynim_emu.so")
-    subprocess.check_call(CXX + [f"-D{d}" for d in defines] +
+    # SYNIM_EMU_CXXFLAGS: extra compiler flags, e.g. "-fsanitize=address,undefined" for a run with libasan preloaded
+    extra = os.environ.get("SYNIM_EMU_CXXFLAGS", "").split()
+    subprocess.check_call(CXX + extra + [f"-D{d}" for d in defines] +
                           ["-I" + HERE, "-I" + gen, "-I" + os.path.join(ROOT, "include"), "-o", lib] + srcs +
                           [os.path.join(HERE, "emu.cpp"), "-ldl"])
     fake = os.path.join(out_dir, "libcublas.so.12")

@@ -412,20 +412,20 @@ def main():
             synim.interaction_matrix_host(geom, h_cube, h_bbox, affines, scales, out_host=h_out, stream=stream, mode=smode)
         try:
             host_step()
+            torch.cuda.synchronize()
         except Exception as exc:        # reported in the line; the device-resident numbers stand on their own
             e2e_error = f"{type(exc).__name__}: {exc}"
         if dist is not None:
             dist.barrier()
-        torch.cuda.synchronize()
         e2e_ms = 0.0
         if e2e_error is None:
             t0 = time.perf_counter()
             try:
                 for _ in range(args.e2e_steps):
                     host_step()
+                torch.cuda.synchronize()
             except Exception as exc:
                 e2e_error = f"{type(exc).__name__}: {exc}"
-            torch.cuda.synchronize()
             e2e_ms = 1e3 * (time.perf_counter() - t0) / args.e2e_steps
         host_in = h_cube.numel() * 4 + (0 if h_bbox is None else h_bbox.numel() * 4)
         if h_bbox is None:
@@ -447,37 +447,42 @@ def main():
     # the multi-layer dictionary of PAPER.md:132-138, end to end through host buffers (optional)
     dictionary = None
     if args.dictionary > 0 and rank == 0:
-        layers = workloads.make_dictionary(n_layers=12, max_modes=args.dictionary)
-        dgeom = synim.create_geometry(layers[0].ny, layers[0].nx, layers[0].wfs)
-        spec = [dict(cube=torch.from_numpy(l.cube).pin_memory(), bbox=torch.from_numpy(l.bbox).pin_memory(),
-                     affines=synim.affines_of(l),
-                     out=torch.empty((l.n_modes, dgeom.num_rows), dtype=torch.float32).pin_memory()) for l in layers]
-        synim.dictionary_host(dgeom, spec, stream=stream)      # warm-up: buffers, module load
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        synim.dictionary_host(dgeom, spec, stream=stream)
-        torch.cuda.synchronize()
-        d_ms = 1e3 * (time.perf_counter() - t0)
-        n_cols = sum(l.n_columns for l in layers)
-        d2h = sum(l.n_modes for l in layers) * dgeom.num_rows * 4
-        from oracle import oracle as O2
-        l0 = layers[-1]
-        pick = np.arange(min(4, l0.n_modes))
-        refd = O2.interaction_matrix(l0, modes=pick)
-        gotd = spec[-1]["out"][: len(pick)].numpy().T.astype(np.float64)
-        dictionary = {"layers": len(layers), "grids": [l.ny for l in layers], "modes_per_layer": [l.n_modes for l in layers],
-                      "columns": n_cols, "ms": d_ms, "columns_per_s": n_cols / (d_ms * 1e-3),
-                      "host_cube_bytes": int(sum(l.cube.nbytes for l in layers)), "d2h_bytes": int(d2h),
-                      "d2h_gbs": d2h / (d_ms * 1e-3) / 1e9,
-                      "top_layer_max_abs_err_vs_oracle": float(np.abs(gotd - refd).max() / np.abs(refd).max()),
-                      "api": "synim_dictionary_host (pinned host buffers, chunks of 64 MB of matrix, two in flight)"}
-        dgeom.destroy()
+        try:
+            layers = workloads.make_dictionary(n_layers=12, max_modes=args.dictionary)
+            dgeom = synim.create_geometry(layers[0].ny, layers[0].nx, layers[0].wfs)
+            spec = [dict(cube=torch.from_numpy(l.cube).pin_memory(), bbox=torch.from_numpy(l.bbox).pin_memory(),
+                         affines=synim.affines_of(l),
+                         out=torch.empty((l.n_modes, dgeom.num_rows), dtype=torch.float32).pin_memory()) for l in layers]
+            synim.dictionary_host(dgeom, spec, stream=stream)      # warm-up: buffers, module load
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            synim.dictionary_host(dgeom, spec, stream=stream)
+            torch.cuda.synchronize()
+            d_ms = 1e3 * (time.perf_counter() - t0)
+            n_cols = sum(l.n_columns for l in layers)
+            d2h = sum(l.n_modes for l in layers) * dgeom.num_rows * 4
+            from oracle import oracle as O2
+            l0 = layers[-1]
+            pick = np.arange(min(4, l0.n_modes))
+            refd = O2.interaction_matrix(l0, modes=pick)
+            gotd = spec[-1]["out"][: len(pick)].numpy().T.astype(np.float64)
+            dictionary = {"layers": len(layers), "grids": [l.ny for l in layers], "modes_per_layer": [l.n_modes for l in layers],
+                          "columns": n_cols, "ms": d_ms, "columns_per_s": n_cols / (d_ms * 1e-3),
+                          "host_cube_bytes": int(sum(l.cube.nbytes for l in layers)), "d2h_bytes": int(d2h),
+                          "d2h_gbs": d2h / (d_ms * 1e-3) / 1e9,
+                          "top_layer_max_abs_err_vs_oracle": float(np.abs(gotd - refd).max() / np.abs(refd).max()),
+                          "api": "synim_dictionary_host (pinned host buffers, chunks of 64 MB of matrix, two in flight)"}
+            dgeom.destroy()
+        except Exception as exc:       # (a side leg: reported, never fatal)
+            dictionary = {"error": f"{type(exc).__name__}: {exc}"}
 
-    times = torch.tensor([float(cold.mean()), e2e[0] if e2e else 0.0, float(warm.mean()), strong_ms], dtype=torch.float64,
-                         device="cuda")
+    # max over ranks (one process: no device work here, so that a side leg that failed above cannot take the line down)
+    times = [float(cold.mean()), e2e[0] if e2e else 0.0, float(warm.mean()), strong_ms]
     if dist is not None:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    cold_ms, e2e_ms, warm_ms, strong_ms = (float(t) for t in times)
+        t = torch.tensor(times, dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        times = [float(x) for x in t]
+    cold_ms, e2e_ms, warm_ms, strong_ms = times
     plan = sharding.weak_scaling_plan(wl.n_columns, world)
 
     if rank == 0:
@@ -533,7 +538,10 @@ def main():
             v1, _, desc1 = oracle_throughput(wl, 6.0, n_threads=1)
             line["cpu_baseline_1thread"] = {"value": v1, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc1}
         print(json.dumps(line), flush=True)
-    geom.destroy()
+    try:
+        geom.destroy()
+    except Exception:
+        pass
     if dist is not None:
         dist.destroy_process_group()
 

@@ -13,12 +13,15 @@ def pytest_configure(config):
 # The GPU run is `pytest -x`: one failure hides every test after it.  So the GPU tests run in the order of how
 # much hardware time the path under test has already seen: first the strip kernel on zonal modes
 # (measured on a B200 in rounds 1 and 2), then everything that (also) goes through the tile kernel, then the host pipeline
-# and the dictionary, and last the paths written after GPU access closed (edge repair, the packed zonal walk, P_opt).
+# and the dictionary, then the paths written after GPU access closed (edge repair, the packed zonal walk, P_opt), and last
+# the -DSYNIM_CHECKS trap build, which drives every one of those paths again (a trap is a device fault: nothing after it
+# in the process can run).
 # The order inside a class is the files' own; tests that need no GPU are not touched.
 _GPU_FIRST = ("test_config1_", "test_config2_", "test_config3_", "test_config4_", "test_compute_bboxes", "test_octagon_")
 _GPU_LATER = (
     ("test_host_", "test_dictionary_host", "test_mode_ranges_through"),
     ("test_edge_repair", "test_packed_zonal", "test_projection_matrix"),
+    ("test_debug_build",),
 )
 
 

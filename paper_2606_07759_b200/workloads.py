@@ -392,3 +392,66 @@ def make_dictionary(n_layers: int = 12, acts_across: int = 66, max_modes: Option
             wfs.append(WfsInput(nsub, npix, pup, val, q))
         out.append(Workload(f"dictionary layer {li} ({h_km:.1f} km, {n}x{n})", 0, n, n, cube, bbox, wfs, keep))
     return out
+
+
+# --------------------------------------------------------------------------
+# seeded random small problems (fuzzing the kernels against the oracle)
+# --------------------------------------------------------------------------
+def random_case(seed: int):
+    """A seeded random SMALL problem and the call options to run it with -> (Workload, options).
+
+    Inputs only, like everything here.  Grids of 32..116 pixels (widths in multiples of 4: the TMA rule of
+    include/synim.h), 1-3 sensors of 1..14 subapertures of 1..40 pixels (at most 120 pixels across) with an annular
+    binary pupil or random fractional weights, rotations over +-180 degrees, anamorphic magnifications 0.6..1.7,
+    shifts of a few pixels, 2-5 modes that are either compact (cut Gaussians of random width and place: the bbox
+    path) or smooth and dense.  ``options``: use_bbox / hint / octagon / ld_pad as in tests/test_gpu_parity.gpu_im,
+    ``mode`` (0 = numerical derivative, 1 = G-tilt) and ``repair`` (None, "binary" or "soft": the modes are then cut by
+    a source-frame mask, Workload.mask, and the repaired entry point applies)."""
+    rng = np.random.default_rng([7759, 2, int(seed)])
+    ny, nx = 4 * int(rng.integers(8, 30)), 4 * int(rng.integers(8, 30))
+    sensors = []
+    for _ in range(int(rng.integers(1, 4))):
+        n_pix = int(rng.choice([1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 16, 23, 31, 40]))
+        n_subap = int(rng.integers(1, max(2, min(14, 120 // n_pix) + 1)))
+        m = n_subap * n_pix
+        pupil = make_pupil(m, rng.uniform(0.8, 1.1) * m, rng.uniform(0.0, 0.3)) if m > 2 else np.ones((m, m), np.float32)
+        if rng.random() < 0.35:      # fractional weights (a soft, unevenly lit pupil)
+            pupil = (pupil * rng.uniform(0.05, 1.0, size=pupil.shape)).astype(np.float32)
+        valid = valid_subaps(pupil, n_subap, n_pix, min_frac=float(rng.uniform(0.15, 0.6)))
+        lit = pupil.astype(np.float64).reshape(n_subap, n_pix, n_subap, n_pix).sum(axis=(1, 3)) > 0
+        valid = (valid.astype(bool) & lit).astype(np.uint8)      # (a valid subaperture with no light is an input error)
+        s = min(ny, nx) / m * rng.uniform(0.6, 1.25)             # source pixels per sensor pixel
+        phys = physical(shift_x=rng.uniform(-3, 3), shift_y=rng.uniform(-3, 3), rot_deg=rng.uniform(-180, 180),
+                        mag_x=rng.uniform(0.6, 1.7), mag_y=rng.uniform(0.6, 1.7), wfs_pitch_src_px=s)
+        if rng.random() < 0.3:
+            phys["mag_y"] = phys["mag_x"]
+        sensors.append(WfsInput(n_subap, n_pix, pupil, valid, phys, slope_scale=float(rng.choice([1.0, 1.0, -0.37, 2.5]))))
+    n_modes = int(rng.integers(2, 6))
+    compact = rng.random() < 0.6
+    if compact:
+        yy, xx = np.mgrid[0:ny, 0:nx].astype(np.float64)
+        cube = np.zeros((n_modes, ny, nx), np.float32)
+        for k in range(n_modes):
+            cx, cy = rng.uniform(-4, nx + 3), rng.uniform(-4, ny + 3)
+            sig, cut = rng.uniform(1.5, 12.0), rng.uniform(1.5, 3.0)
+            r2 = (xx - cx) ** 2 + (yy - cy) ** 2
+            z = rng.normal() * np.exp(-0.5 * r2 / sig ** 2)
+            z[r2 > (cut * sig) ** 2] = 0.0
+            if k == n_modes - 1 and rng.random() < 0.25:
+                z[:] = 0.0                                           # an empty mode
+            cube[k] = z.astype(np.float32)
+        bbox = tight_bboxes(cube)
+    else:
+        cube, bbox = random_smooth_cube(n_modes, ny, nx, 1000 + int(seed)), None
+    wl = Workload(f"random case {seed}", 0, ny, nx, cube, bbox, sensors)
+    opts = dict(use_bbox=bool(rng.random() < 0.8), hint=bool(rng.random() < 0.7), octagon=bool(rng.random() < 0.7),
+                ld_pad=int(rng.choice([0, 0, 3])), mode=int(rng.random() < 0.25), repair=None)
+    if opts["mode"] == 0 and rng.random() < 0.35:
+        import scipy.ndimage as ndi
+        opts["repair"] = "soft" if rng.random() < 0.5 else "binary"
+        blob = ndi.gaussian_filter(rng.normal(size=(ny, nx)), 5.0)
+        mask = (blob > np.quantile(blob, rng.uniform(0.1, 0.4))).astype(np.float64)
+        if opts["repair"] == "soft":
+            mask = np.clip(ndi.gaussian_filter(mask, 0.8) * 1.3, 0.0, 1.0)
+        wl = masked(wl, mask.astype(np.float32))
+    return wl, opts

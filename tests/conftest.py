@@ -21,6 +21,7 @@ _GPU_FIRST = ("test_config1_", "test_config2_", "test_config3_", "test_config4_"
 _GPU_LATER = (
     ("test_host_", "test_dictionary_host", "test_mode_ranges_through"),
     ("test_edge_repair", "test_packed_zonal", "test_projection_matrix"),
+    ("test_seeded_random_cases",),
     ("test_debug_build",),
 )
 

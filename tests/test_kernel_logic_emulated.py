@@ -50,7 +50,7 @@ def check(got, ref, wl, tol=TOL):
             err = np.abs(g - r)
             assert (err <= tol * cmax[None, :] + fl[None, :]).all()
             assert (np.linalg.norm(g - r, axis=0) <= tol * np.linalg.norm(r, axis=0) + fl * np.sqrt(r.shape[0])).all()
-            live = cmax >= 100.0 * floor
+            live = (cmax >= 100.0 * floor) & (cmax > 0.0)
             if live.any():
                 worst = max(worst, float((err.max(axis=0)[live] / cmax[live]).max()))
         r0 = r1
@@ -282,3 +282,28 @@ def test_two_gloo_ranks_shard_the_modes_through_the_kernels(emu):
         assert (b, e_) == ranges[rank]
         assert np.array_equal(full, whole)
     check(whole.T.astype(np.float64), O.interaction_matrix(wl), wl)
+
+
+def test_seeded_random_cases_against_the_oracle(emu):
+    """Fuzzing, committed: the first cases of workloads.random_case (random grids, 1-3 sensors of 1..14 subapertures of
+    1..40 pixels with binary or fractional pupils, rotations over +-180 degrees, anamorphic magnifications, compact or
+    dense modes, every call option, both estimators, edge repair with binary and soft masks, sensors without a valid
+    subaperture, empty modes) through the emulated library, each against the oracle at the north_star bar.
+    SYNIM_FUZZ_CASES widens the campaign (default 64; the same seeds run on the GPU in tests/test_gpu_parity.py)."""
+    n = int(os.environ.get("SYNIM_FUZZ_CASES", "64"))
+    worst, kinds = 0.0, set()
+    for seed in range(n):
+        wl, o = W.random_case(seed)
+        rep = o.pop("repair")
+        mask = wl.mask if rep else None
+        ref = O.interaction_matrix(wl, mode=O.GTILT if o["mode"] else O.ND, repair_mask=mask)
+        try:
+            worst = max(worst, check(emu.interaction_matrix(wl, mask=mask, **o), ref, wl))
+        except AssertionError as exc:
+            raise AssertionError(f"random case {seed} ({o}, repair={rep})") from exc
+        kinds.add((wl.bbox is None or not o["use_bbox"], o["mode"], rep))
+    print(f"{n} random cases, worst elementwise error {worst:.2e} of the column maximum")
+    assert worst <= TOL
+    if n >= 64:      # the campaign reaches every path: compact / dense x estimator x repair
+        assert {(False, 0, None), (True, 0, None), (False, 1, None), (True, 1, None)} <= kinds
+        assert any(k[2] == "binary" for k in kinds) and any(k[2] == "soft" for k in kinds)

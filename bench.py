@@ -24,6 +24,9 @@ source-frame mask; --dictionary M adds the 12-layer dictionary of PAPER.md:132 (
 synim_dictionary_host under config.dictionary.
 --extra (default "2,4,5,3r,3g,3p"): at N=1 the line also carries, under config.other_configs, short device-resident runs
 of the other configurations, each in its own process.
+config.ablation (and other_configs[*].ablation; --no-ablate to skip): after everything else, a few cold steps each of a plain
+fill of the matrix (the write stream alone), half the modes and one wave of CTAs, and every class of sensors on its own --
+what a step's time is made of, measured on the box that ran the line.
 --impl reference times the oracle only (rank 0; other ranks exit).  N > 1: every rank holds its own
 workload of the same shape (independent problems, no data-path collective): weak scaling.
 """
@@ -191,11 +194,60 @@ def other_configs(spec: str) -> dict:
                         "algorithmic_bytes": d["roofline"]["algorithmic_bytes"]["total"], "kernel": d["roofline"]["kernel"],
                         "gpu_launches": d["gpu_launches"], "parity_spot_check": d["parity_spot_check"],
                         "clocks": d["clocks"], "slope_mode": d["config"].get("slope_mode"),
-                        "edge_repair": d["config"].get("edge_repair"),
+                        "edge_repair": d["config"].get("edge_repair"), "ablation": d["config"].get("ablation"),
                         "packed_zonal_walk": tag.endswith("p")}
         except Exception as exc:
             out[tag] = {"error": f"{type(exc).__name__}: {exc}"}
     return out
+
+
+def ablate(synim, wl, geom, cube, bbox, diag, bmax, affines, scales, out, scratch, stream, smode, full_ms, k=5):
+    """Measured decomposition of a step (cold-L2 protocol, mean of k steps each): the write stream alone, fewer modes
+    (is the grid's tail or the launch what is paid for?), and every class of sensors on its own."""
+    import torch
+
+    def cold_ms(fn):
+        fn(); fn()
+        e0 = [torch.cuda.Event(enable_timing=True) for _ in range(k)]
+        e1 = [torch.cuda.Event(enable_timing=True) for _ in range(k)]
+        for i in range(k):
+            scratch.fill_(i & 0xff)
+            e0[i].record(stream); fn(); e1[i].record(stream)
+        torch.cuda.synchronize()
+        return float(np.mean([e0[i].elapsed_time(e1[i]) for i in range(k)]))
+
+    def run(g, n, o, aff, sc):
+        synim.interaction_matrix(g, cube[:n], None if bbox is None else bbox[:n], aff, sc, out=o, bbox_max=bmax, stream=stream,
+                                 diag=None if diag is None else diag[:n], mode=smode)
+
+    res = {"protocol": f"cold L2, mean of {k} steps each", "full_step_ms": full_ms,
+           "im_fill_ms": cold_ms(lambda: out.zero_()),
+           "im_fill_note": "torch fill of the whole matrix buffer: the write stream alone, no sampling"}
+    n = wl.n_modes
+    counts = {"half_modes": n // 2}
+    if bbox is not None:
+        counts["one_wave_1036_ctas"] = min(n, 148 * 7)      # synim_strip_kernel: one CTA per mode, 7 CTAs per SM
+    res["fewer_modes"] = {tag: {"n_modes": c, "ms": cold_ms(lambda c=c: run(geom, c, out[:c], affines, scales))}
+                          for tag, c in counts.items() if 0 < c < n}
+    # sensors: every class (same subaperture grid) on its own, and the first sensor alone
+    classes = {}
+    for i, w in enumerate(wl.wfs):
+        classes.setdefault((w.n_subap, w.n_pix), []).append(i)
+    groups = {f"{ns}x{ns} subapertures of {npx} px ({len(ix)} sensors)": ix for (ns, npx), ix in classes.items() if len(classes) > 1}
+    if len(wl.wfs) > 1:
+        groups["first sensor alone"] = [0]
+        groups["second sensor alone"] = [1]
+    res["sensors"] = {}
+    for tag, ix in groups.items():
+        sub = [wl.wfs[i] for i in ix]
+        g = synim.create_geometry(wl.ny, wl.nx, sub)
+        o = torch.empty((n, g.num_rows), dtype=torch.float32, device=out.device)
+        aff, sc = [affines[i] for i in ix], [scales[i] for i in ix]
+        res["sensors"][tag] = {"columns": n * len(ix), "im_bytes": int(o.numel() * 4), "ms": cold_ms(lambda: run(g, n, o, aff, sc))}
+        torch.cuda.synchronize()
+        g.destroy()
+        del o
+    return res
 
 
 def run_reference(args, rank: int):
@@ -242,6 +294,10 @@ def main():
                          "own process, reported under config.other_configs ('3r' = config 3 with edge repair, '3g' = config 3 "
                          "with the G-tilt estimator, '3p' = config 3 through the opt-in packed zonal walk, SYNIM_ZONAL_PACKED=1; "
                          "'none' to skip)")
+    ap.add_argument("--no-ablate", action="store_true",
+                    help="skip config.ablation: after the timed run, a few cold steps each of (a) a plain fill of the matrix "
+                         "(the write stream alone), (b) half the modes, and one wave of CTAs for zonal modes, (c) every class of "
+                         "sensors (and a single sensor) on its own -- what the step time is made of, measured, not inferred")
     ap.add_argument("--slope-mode", default="nd", choices=["nd", "gtilt"],
                     help="nd = the paper's numerical-derivative engine (the metric); gtilt = the comparison estimator")
     args = ap.parse_args()
@@ -476,6 +532,15 @@ def main():
         except Exception as exc:       # (a side leg: reported, never fatal)
             dictionary = {"error": f"{type(exc).__name__}: {exc}"}
 
+    # what the step time is made of (N = 1; the last device work of the run; a side leg: reported, never fatal)
+    ablation = None
+    if world == 1 and not args.no_ablate and not args.repair:
+        try:
+            ablation = ablate(synim, wl, geom, cube, bbox, diag, bmax, affines, scales, out, scratch, stream, smode,
+                              float(cold.mean()))
+        except Exception as exc:
+            ablation = {"error": f"{type(exc).__name__}: {exc}"}
+
     # max over ranks (one process: no device work here, so that a side leg that failed above cannot take the line down)
     times = [float(cold.mean()), e2e[0] if e2e else 0.0, float(warm.mean()), strong_ms]
     if dist is not None:
@@ -500,6 +565,8 @@ def main():
                  "first_call": first_call}
         if dictionary:
             extra["dictionary"] = dictionary
+        if ablation:
+            extra["ablation"] = ablation
         if args.repair:
             extra["edge_repair"] = "synim_interaction_matrix_repaired, threshold 0.999999, modes cut by a round source-frame mask"
         if world > 1:

@@ -658,9 +658,14 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
                 p.tab_floats = (tab + 3) & ~3;
                 p.tiles_total = tiles;
                 const size_t tsmem = sizeof(float) * ((size_t)box_floats + (size_t)p.tab_floats) + sizeof(int) * (size_t)(p.tab_floats / 2);
-                for (int m0 = 0; m0 < n_modes; m0 += 65535) {   // grid.y holds the modes
+                int batch = 65535;   // grid.y holds the modes
+                if (const char *env = std::getenv("SYNIM_TILE_BATCH_MODES")) {   // test knob: smaller batches
+                    const int v = std::atoi(env);
+                    if (v >= 1 && v < batch) batch = v;
+                }
+                for (int m0 = 0; m0 < n_modes; m0 += batch) {
                     synim::ImParams q = p;
-                    q.n_modes = std::min(65535, n_modes - m0);
+                    q.n_modes = std::min(batch, n_modes - m0);
                     q.out = d_out + (size_t)m0 * (size_t)ld;
                     if (m0 > 0) {   // the descriptors address modes from the cube's start: re-encode on the batch
                         const float *sub = d_influence + (size_t)m0 * (size_t)cube_ny * (size_t)cube_nx;

@@ -244,6 +244,16 @@ def test_more_than_sixteen_sensors_take_a_second_launch(S):
     assert_parity(gpu_im(S, wl, mode=S.SLOPES_GTILT, ld_pad=5), O.interaction_matrix(wl, mode=O.GTILT), wl)
 
 
+def test_more_than_65535_dense_modes_take_a_second_batch(S):
+    """The tile kernel keeps the modes in grid.y (<= 65535): a larger cube goes in batches, each with descriptors
+    re-encoded on its part of the cube and its own part of the matrix (synim_api.cu, run_interaction_matrix)."""
+    n = 65700
+    cube = np.random.default_rng(5).normal(size=(n, 8, 8)).astype(np.float32)
+    s = [W.WfsInput(2, 4, np.ones((8, 8), np.float32), np.ones((2, 2), np.uint8), W.physical(rot_deg=7.0, shift_x=0.3))]
+    wl = W.Workload(f"{n} small dense modes", 0, 8, 8, cube, None, s)
+    assert_parity(gpu_im(S, wl), O.interaction_matrix(wl), wl)
+
+
 def test_dense_modes_with_padding_rows(S):
     """Dense modes into a matrix with ld > rows (padding rows must stay untouched), aligned and not."""
     wl = W.make_config(5, max_modes=4)

@@ -101,6 +101,19 @@ def test_tile_kernel_dense_modes(emu):
         check(emu.interaction_matrix(wl), O.interaction_matrix(wl), wl)
 
 
+def test_tile_kernel_batches_of_modes(emu, monkeypatch):
+    """grid.y holds the modes of the tile kernel, at most 65535 of them: larger cubes are cut into batches, each with
+    descriptors re-encoded on its part of the cube and its own part of the matrix.  The emulation of a CTA costs
+    milliseconds, so the batch size comes down through the library's test knob (tests/test_gpu_parity.py runs the real
+    65,700 modes)."""
+    monkeypatch.setenv("SYNIM_TILE_BATCH_MODES", "300")
+    cube = np.random.default_rng(5).normal(size=(700, 8, 8)).astype(np.float32)
+    s = [W.WfsInput(2, 4, np.ones((8, 8), np.float32), np.ones((2, 2), np.uint8), W.physical(rot_deg=7.0, shift_x=0.3))]
+    wl = W.Workload("700 small dense modes", 0, 8, 8, cube, None, s)
+    check(emu.interaction_matrix(wl, count_stores=True), O.interaction_matrix(wl), wl)
+    assert (emu.store_counts == 1).all()
+
+
 def test_edge_repair_in_both_kernels(emu):
     wl = W.masked(W.make_config(1, max_modes=20), W.make_pupil(80, 80.0, 0.14))
     ref = O.interaction_matrix(wl, repair_mask=wl.mask)

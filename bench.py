@@ -22,7 +22,7 @@ workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators 
 --repair times synim_interaction_matrix_repaired (edge repair) on the config's modes cut by a
 source-frame mask; --dictionary M adds the 12-layer dictionary of PAPER.md:132 (M modes per layer) through
 synim_dictionary_host under config.dictionary.
---extra (default "2,4,5,3r,3g,3p"): at N=1 the line also carries, under config.other_configs, short device-resident runs
+--extra (default "2,4,5,3r,3g,3p,4p"): at N=1 the line also carries, under config.other_configs, short device-resident runs
 of the other configurations, each in its own process.
 config.ablation (and other_configs[*].ablation; --no-ablate to skip): after everything else, a few cold steps each of a plain
 fill of the matrix (the write stream alone), half the modes and one wave of CTAs, and every class of sensors on its own --
@@ -289,10 +289,10 @@ def main():
     ap.add_argument("--dictionary", type=int, default=0, metavar="MODES_PER_LAYER",
                     help="also run the 12-layer dictionary of PAPER.md:132 (workloads.make_dictionary, this many modes per "
                          "layer) through synim_dictionary_host and report it under config.dictionary")
-    ap.add_argument("--extra", default="2,4,5,3r,3g,3p",
+    ap.add_argument("--extra", default="2,4,5,3r,3g,3p,4p",
                     help="at N=1, after the timed run: short device-resident runs of these other configurations, each in its "
                          "own process, reported under config.other_configs ('3r' = config 3 with edge repair, '3g' = config 3 "
-                         "with the G-tilt estimator, '3p' = config 3 through the opt-in packed zonal walk, SYNIM_ZONAL_PACKED=1; "
+                         "with the G-tilt estimator, '3p' / '4p' = config 3 / 4 through the opt-in packed zonal walk, SYNIM_ZONAL_PACKED=1; "
                          "'none' to skip)")
     ap.add_argument("--no-ablate", action="store_true",
                     help="skip config.ablation: after the timed run, a few cold steps each of (a) a plain fill of the matrix "

@@ -83,7 +83,7 @@ def _check_block(g, r, tol, floor, stats):
     if live.any():
         stats["l2"] = max(stats["l2"], float((np.linalg.norm(g - r, axis=0)[live] / nrm[live]).max()))
         stats["el"] = max(stats["el"], float((err.max(axis=0)[live] / cmax[live]).max()))
-    stats["floored"] += int(dead.sum())
+    stats["floored"] += int((dead & (cmax > 0.0)).sum())
     stats["columns"] += int(dead.size)
     assert (g[:, cmax == 0] == 0).all(), "a (mode, WFS) column the oracle gives as exactly 0 is not 0"
     # Skipping is exact (R15): wherever the oracle is exactly 0 the GPU is exactly 0, except on the

@@ -140,7 +140,7 @@ def test_edge_repair_in_both_kernels(emu):
 
 def test_packed_zonal_walk_opt_in(emu, monkeypatch):
     monkeypatch.setenv("SYNIM_ZONAL_PACKED", "1")
-    for cfg, n in ((1, 30), (3, 6)):
+    for cfg, n in ((1, 30), (3, 6), (4, 6)):       # (config 4: the LGS launch packed, the giant NGS subapertures as ever)
         wl = W.make_config(cfg, max_modes=n)
         check(emu.interaction_matrix(wl), O.interaction_matrix(wl), wl)
 

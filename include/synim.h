@@ -43,7 +43,7 @@ extern "C" {
 #endif
 
 #define SYNIM_VERSION_MAJOR 0
-#define SYNIM_VERSION_MINOR 2
+#define SYNIM_VERSION_MINOR 3
 
 typedef struct synim_geometry synim_geometry; /* opaque, library-owned */
 
@@ -169,6 +169,19 @@ synim_status synim_compute_bboxes(const float *d_influence, int32_t n_modes, int
 /* Largest bbox width / height (HOST out); synchronises `stream`. */
 synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *max_w, int32_t *max_h,
                                void *stream);
+
+/* One-shot form with north_star's argument list (BASELINE.json; "a flat convenience wrapper ... may
+ * wrap create -> compute -> destroy"): influence cube, per-sensor pupil mask + subaperture grid + valid mask (grids),
+ * per-sensor composite matrices (affine), out IM [2 * sum_w n_valid_w][n_modes] column-major.  All buffers DEVICE except
+ * grids[w].valid_mask and affine (HOST), exactly as in the calls it wraps:
+ *   synim_create_geometry -> (compact != 0: synim_compute_bboxes + synim_bbox_extent, so that empty tiles are skipped;
+ *   compact == 0: dense modes) -> synim_interaction_matrix -> synim_destroy.
+ * ld >= 2 * sum_w n_valid_w, which the caller derives from its own valid masks; rows_out (may be NULL) receives it.
+ * The supports live in a stream-ordered allocation of 32 * n_modes bytes for the duration of the call.  SYNCHRONISES the
+ * device before returning (the geometry it built is freed).  For repeated use keep a geometry and call the pieces. */
+synim_status synim_interaction_matrix_flat(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx, int32_t n_wfs,
+                                           const synim_wfs_grid *grids, const synim_wfs_affine *affine, int32_t compact,
+                                           synim_slope_mode mode, float *d_out, int64_t ld, int64_t *rows_out, void *stream);
 
 /* Convenience wrapper with HOST buffers, for one-shot use and end-to-end timing: brings the cube to
  * the device, runs synim_interaction_matrix, copies the IM back and synchronises.  h_out is column-major

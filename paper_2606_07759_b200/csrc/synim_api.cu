@@ -766,6 +766,35 @@ synim_status synim_bbox_extent(const int32_t *d_bbox, int32_t n_modes, int32_t *
     return SYNIM_OK;
 }
 
+synim_status synim_interaction_matrix_flat(const float *d_influence, int32_t n_modes, int32_t ny, int32_t nx, int32_t n_wfs,
+                                           const synim_wfs_grid *grids, const synim_wfs_affine *affine, int32_t compact,
+                                           synim_slope_mode mode, float *d_out, int64_t ld, int64_t *rows_out, void *stream)
+{
+    if (rows_out) *rows_out = -1;
+    if (!affine || n_modes < 0) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix_flat: NULL affine or n_modes < 0");
+    synim_geometry *g = nullptr;
+    synim_status st = synim_create_geometry(ny, nx, n_wfs, grids, stream, &g);
+    if (st != SYNIM_OK) return st;
+    if (rows_out) *rows_out = g->rows;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int32_t *d_sup = nullptr;   // [n_modes][4] bboxes, then [n_modes][4] diagonal extents
+    int32_t bw = 0, bh = 0;
+    if (compact && n_modes > 0) {
+        cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&d_sup), sizeof(int32_t) * 8 * (size_t)n_modes, s);
+        if (e != cudaSuccess) st = cuda_fail(e, "cudaMallocAsync(supports)");
+        if (st == SYNIM_OK) st = synim_compute_bboxes(d_influence, n_modes, ny, nx, d_sup, d_sup + 4 * (size_t)n_modes, stream);
+        if (st == SYNIM_OK) st = synim_bbox_extent(d_sup, n_modes, &bw, &bh, stream);
+    }
+    if (st == SYNIM_OK)
+        st = run_interaction_matrix(g, d_influence, ny, nx, nullptr, n_modes, d_sup, d_sup ? d_sup + 4 * (size_t)n_modes : nullptr, bw, bh,
+                                    affine, mode, d_out, ld, stream);
+    if (d_sup) cudaFreeAsync(d_sup, s);
+    const cudaError_t e = cudaDeviceSynchronize();   // the geometry's maps are in use until the launches have drained
+    synim_destroy(g);
+    if (st == SYNIM_OK && e != cudaSuccess) st = cuda_fail(e, "synim_interaction_matrix_flat");
+    return st;
+}
+
 // The pipeline behind both host entry points.  The modes of every layer are cut into chunks; chunk k is packed on the
 // host (compact supports only) while chunk k-1 runs and chunk k-2 goes home:
 //     host: pack k | s_compute: H2D k, kernel k | s_copy: D2H k        (two buffers of everything, events between)

@@ -21,7 +21,8 @@ SLOPES_ND, SLOPES_GTILT = 0, 1
 
 #: every symbol include/synim.h declares
 EXPORTS = ("synim_compose_affine", "synim_create_geometry", "synim_num_rows", "synim_num_valid",
-           "synim_row_offset", "synim_interaction_matrix", "synim_interaction_matrix_repaired", "synim_compute_bboxes",
+           "synim_row_offset", "synim_interaction_matrix", "synim_interaction_matrix_repaired",
+           "synim_interaction_matrix_flat", "synim_compute_bboxes",
            "synim_bbox_extent",
            "synim_interaction_matrix_host", "synim_dictionary_host", "synim_projection_matrix", "synim_destroy", "synim_last_error", "synim_version",
            "synim_launch_count")
@@ -90,6 +91,9 @@ def lib() -> ctypes.CDLL:
         L.synim_interaction_matrix_repaired.restype = ctypes.c_int
         L.synim_interaction_matrix_repaired.argtypes = [vp, vp, i32, vp, vp, i32, i32, ctypes.POINTER(WfsAffine), vp,
                                                         ctypes.c_double, vp, i64, vp]
+        L.synim_interaction_matrix_flat.restype = ctypes.c_int
+        L.synim_interaction_matrix_flat.argtypes = [vp, i32, i32, i32, i32, ctypes.POINTER(WfsGrid), ctypes.POINTER(WfsAffine),
+                                                    i32, ctypes.c_int, vp, i64, ctypes.POINTER(i64), vp]
         L.synim_compute_bboxes.restype = ctypes.c_int
         L.synim_compute_bboxes.argtypes = [vp, i32, i32, i32, vp, vp, vp]
         L.synim_bbox_extent.restype = ctypes.c_int
@@ -300,6 +304,35 @@ def interaction_matrix(geom: Geometry, cube, bbox, affines: Sequence[Sequence[fl
         return out
     _check(lib().synim_interaction_matrix(geom._h, cube.data_ptr(), n, bptr, dptr, int(bbox_max[0]), int(bbox_max[1]),
                                           arr, int(mode), out.data_ptr(), ld, _stream_ptr(stream)))
+    return out
+
+
+def interaction_matrix_flat(cube, wfs: Sequence, affines: Sequence[Sequence[float]], scales: Optional[Sequence[float]] = None,
+                            compact: bool = True, mode: int = SLOPES_ND, stream=None):
+    """synim_interaction_matrix_flat: the one-shot call with north_star's argument list (cube, per-sensor pupil mask,
+    subaperture grid and valid mask, per-sensor composite matrices) -> CUDA float32 [n_modes][rows].  ``wfs`` as for
+    ``Geometry``; the library builds and frees its own geometry and synchronises the device."""
+    import torch
+    assert cube.is_cuda and cube.dtype == torch.float32 and cube.is_contiguous() and cube.dim() == 3
+    n, ny, nx = (int(v) for v in cube.shape)
+    grids = (WfsGrid * len(wfs))()
+    keep, rows = [], 0
+    for k, w in enumerate(wfs):
+        valid = np.ascontiguousarray(w.valid, dtype=np.uint8)
+        pupil = w.pupil if isinstance(w.pupil, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(w.pupil, dtype=np.float32))
+        pupil = pupil.to(device="cuda", dtype=torch.float32).contiguous()
+        keep.append((valid, pupil))
+        grids[k].n_subap, grids[k].n_pix = int(w.n_subap), int(w.n_pix)
+        grids[k].valid_mask = valid.ctypes.data
+        grids[k].d_pupil = pupil.data_ptr()
+        rows += 2 * int(np.count_nonzero(valid))
+    out = torch.empty((n, max(rows, 1)), dtype=torch.float32, device=cube.device)[:, :rows]
+    got = ctypes.c_int64(-1)
+    _check(lib().synim_interaction_matrix_flat(cube.data_ptr(), n, ny, nx, len(wfs), grids, _affine_array(affines, scales),
+                                               1 if compact else 0, int(mode), out.data_ptr(), int(out.stride(0)),
+                                               ctypes.byref(got), _stream_ptr(stream)))
+    assert got.value == rows
+    del keep
     return out
 
 

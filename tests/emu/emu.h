@@ -149,6 +149,7 @@ static inline cudaError_t cudaMemset2DAsync(void *d, size_t pitch, int v, size_t
     return cudaSuccess;
 }
 static inline cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSuccess; }
+static inline cudaError_t cudaDeviceSynchronize() { return cudaSuccess; }
 typedef void *cudaEvent_t;
 enum { cudaStreamNonBlocking = 1, cudaEventDisableTiming = 2 };
 static inline cudaError_t cudaStreamCreateWithFlags(cudaStream_t *s, int) { *s = (cudaStream_t)malloc(8); return cudaSuccess; }

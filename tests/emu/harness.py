@@ -56,6 +56,8 @@ class Emu:
         L.synim_interaction_matrix.argtypes = [vp, vp, i32, vp, vp, i32, i32, ctypes.POINTER(S.WfsAffine), ctypes.c_int, vp, i64, vp]
         L.synim_interaction_matrix_repaired.argtypes = [vp, vp, i32, vp, vp, i32, i32, ctypes.POINTER(S.WfsAffine), vp,
                                                         ctypes.c_double, vp, i64, vp]
+        L.synim_interaction_matrix_flat.argtypes = [vp, i32, i32, i32, i32, ctypes.POINTER(S.WfsGrid), ctypes.POINTER(S.WfsAffine),
+                                                    i32, ctypes.c_int, vp, i64, ctypes.POINTER(i64), vp]
         L.synim_compute_bboxes.argtypes = [vp, i32, i32, i32, vp, vp, vp]
         L.synim_bbox_extent.argtypes = [vp, i32, ctypes.POINTER(i32), ctypes.POINTER(i32), vp]
         L.synim_interaction_matrix_host.argtypes = [vp, vp, i32, vp, ctypes.POINTER(S.WfsAffine), ctypes.c_int, vp, vp]
@@ -106,6 +108,30 @@ class Emu:
         h = ctypes.c_void_p()
         self.chk(self.L.synim_create_geometry(ny, nx, n, grids, None, ctypes.byref(h)))
         return h, keep
+
+    def interaction_matrix_flat(self, wl, compact=True, mode=0):
+        """synim_interaction_matrix_flat (create -> supports -> matrix -> destroy in one call) -> float64 [rows][n_modes]."""
+        L = self.L
+        n = len(wl.wfs)
+        grids = (S.WfsGrid * n)()
+        keep = []
+        for k, w in enumerate(wl.wfs):
+            valid = np.ascontiguousarray(w.valid, dtype=np.uint8)
+            pupil = self.reg(np.ascontiguousarray(w.pupil, dtype=np.float32).copy())
+            keep.append((valid, pupil))
+            grids[k].n_subap, grids[k].n_pix = int(w.n_subap), int(w.n_pix)
+            grids[k].valid_mask = valid.ctypes.data
+            grids[k].d_pupil = pupil.ctypes.data
+        cube = self.reg(np.ascontiguousarray(wl.cube, dtype=np.float32))
+        out = self.reg(np.full((wl.n_modes, wl.n_rows), np.nan, np.float32))
+        arr = S._affine_array(self.affines(wl.wfs), [w.slope_scale for w in wl.wfs])
+        rows = ctypes.c_int64(-1)
+        self.chk(L.synim_interaction_matrix_flat(cube.ctypes.data, wl.n_modes, wl.ny, wl.nx, n, grids, arr, 1 if compact else 0, mode,
+                                                 out.ctypes.data, wl.n_rows, ctypes.byref(rows), None))
+        assert rows.value == wl.n_rows
+        res = out.T.astype(np.float64)
+        assert np.isfinite(res).all(), "unwritten IM elements"
+        return res
 
     def interaction_matrix(self, wl, use_bbox=True, ld_pad=0, hint=True, octagon=True, mode=0, affines=None, scales=None,
                            mask=None, threshold=0.999999, count_stores=False):

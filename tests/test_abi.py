@@ -29,7 +29,7 @@ def test_library_exports_every_declared_symbol(lib):
     assert declared == set(synim.EXPORTS)
     for name in declared:
         assert getattr(lib, name) is not None
-    assert synim.version() == 2
+    assert synim.version() == 3
 
 
 def test_compose_affine_matches_the_oracles_independent_composition(lib):

@@ -543,6 +543,21 @@ def test_dictionary_host_streams_layers_with_their_own_grids(S, monkeypatch):
     geom.destroy()
 
 
+def test_flat_one_shot_entry_point(S):
+    """synim_interaction_matrix_flat (north_star's argument list: create -> supports -> matrix -> destroy in one call)
+    gives the matrix of the piecewise calls bit for bit, and meets the bar on its own."""
+    import torch
+    for cfg, n in ((1, None), (4, 12)):
+        wl = W.make_config(cfg, max_modes=n)
+        cube = torch.from_numpy(wl.cube).cuda()
+        aff, sc = S.affines_of(wl), [w.slope_scale for w in wl.wfs]
+        flat = S.interaction_matrix_flat(cube, wl.wfs, aff, sc).cpu().numpy().T
+        assert np.array_equal(flat, gpu_im(S, wl))
+        assert_parity(flat, O.interaction_matrix(wl), wl)
+        dense = S.interaction_matrix_flat(cube, wl.wfs, aff, sc, compact=False).cpu().numpy().T
+        assert np.array_equal(dense, gpu_im(S, wl, use_bbox=False))
+
+
 def test_mode_ranges_through_the_library_concatenate_to_the_unsharded_matrix(S):
     """the mode axis shards with no exchange.  The ranges of sharding.partition_modes go through
     synim_interaction_matrix one by one (as the ranks of a job would, each on its slice of the cube and its block of

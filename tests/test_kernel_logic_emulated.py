@@ -83,6 +83,17 @@ def test_strip_kernel_zonal_modes(emu):
     check(emu.interaction_matrix(wl, hint=False), O.interaction_matrix(wl), wl)
 
 
+def test_flat_one_shot_entry_point(emu):
+    """synim_interaction_matrix_flat (north_star's argument list: create -> supports -> matrix -> destroy) gives the
+    matrix of the piecewise calls bit for bit, compact and dense, both estimators."""
+    wl = W.make_config(1, max_modes=16)
+    assert np.array_equal(emu.interaction_matrix_flat(wl), emu.interaction_matrix(wl))
+    assert np.array_equal(emu.interaction_matrix_flat(wl, compact=False), emu.interaction_matrix(wl, use_bbox=False))
+    check(emu.interaction_matrix_flat(wl, mode=1), O.interaction_matrix(wl, mode=O.GTILT), wl)
+    wl = W.make_config(4, max_modes=4)
+    check(emu.interaction_matrix_flat(wl), O.interaction_matrix(wl), wl)
+
+
 def test_tile_kernel_dense_modes(emu):
     """Tiles of the WFS grid: narrow last strips (the lanes beyond a strip's halo column once read outside the staged box
     -- the emulator aborts on such an access), partially lit units, skipped units, both estimators, padding rows."""

@@ -85,3 +85,49 @@ def test_every_planted_mistake_fails_a_pin(tmp_path):
         survived = list(pool.map(_survives, jobs))
     alive = [MUTATIONS[i][0] for i, s in enumerate(survived) if s]
     assert not alive, f"mutants no pin catches: {alive}"
+
+
+# The projection-matrix oracle is numpy code in oracle/oracle.py: the same game, with the mutated module
+# installed as oracle.oracle in a child interpreter before the pins (tests/test_oracle_projection_pins.py) are collected.
+PY_MUTATIONS = [
+    ("popt: regulariser subtracted", "+ float(lam) * np.eye(p_dm.shape[1])", "- float(lam) * np.eye(p_dm.shape[1])"),
+    ("popt: regulariser ignored", "+ float(lam) * np.eye(p_dm.shape[1])", "+ 0.0 * np.eye(p_dm.shape[1])"),
+    ("popt: no inverse", "return np.linalg.solve(g, p_dm.T @ p_layer)", "return g @ (p_dm.T @ p_layer)"),
+    ("popt: direction weights not square-rooted", "float(np.sqrt(w[d])) *", "float(w[d]) *"),
+    ("popt: pupil weighting dropped", "(pupil * resample(cube[m], mp, maps[d])).ravel()", "(resample(cube[m], mp, maps[d])).ravel()"),
+    ("popt: every direction seen through the first map", "resample(cube[m], mp, maps[d])", "resample(cube[m], mp, maps[0])"),
+]
+
+_CHILD = r"""
+import sys, types
+root, old, new = sys.argv[1], sys.argv[2], sys.argv[3]
+sys.path.insert(0, root)
+import oracle as pkg
+path = root + "/oracle/oracle.py"
+src = open(path).read()
+assert old in src, "mutation no longer applies to oracle/oracle.py"
+mod = types.ModuleType("oracle.oracle")
+mod.__file__ = path
+mod.__package__ = "oracle"
+sys.modules["oracle.oracle"] = mod
+exec(compile(src.replace(old, new, 1), path, "exec"), mod.__dict__)
+pkg.oracle = mod
+import pytest
+sys.exit(pytest.main([root + "/tests/test_oracle_projection_pins.py", "-x", "-q", "-p", "no:cacheprovider"]))
+"""
+
+
+def _py_survives(m):
+    name, old, new = m
+    res = subprocess.run([sys.executable, "-c", _CHILD, ROOT, old, new], cwd=ROOT, capture_output=True, text=True, timeout=600)
+    assert "no longer applies" not in res.stderr, name
+    return res.returncode == 0
+
+
+@pytest.mark.timeout(600)
+def test_every_planted_mistake_in_the_projection_oracle_fails_a_pin():
+    assert _py_survives(("control", "written out as the paper gives it", "written out as the paper gives it "))
+    with ThreadPoolExecutor(max_workers=min(6, os.cpu_count() or 1)) as pool:
+        survived = list(pool.map(_py_survives, PY_MUTATIONS))
+    alive = [PY_MUTATIONS[i][0] for i, s in enumerate(survived) if s]
+    assert not alive, f"mutants no pin catches: {alive}"

@@ -22,7 +22,7 @@ workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators 
 --repair times synim_interaction_matrix_repaired (edge repair) on the config's modes cut by a
 source-frame mask; --dictionary M adds the 12-layer dictionary of PAPER.md:132 (M modes per layer) through
 synim_dictionary_host under config.dictionary.
---extra (default "2,4,5,3r,3g,3p,4p"): at N=1 the line also carries, under config.other_configs, short device-resident runs
+--extra (default "5,4,2,3p,4p,3g,3r", most wanted first): at N=1 the line also carries, under config.other_configs, short device-resident runs
 of the other configurations, each in its own process.
 config.ablation (and other_configs[*].ablation; --no-ablate to skip): after everything else, a few cold steps each of a plain
 fill of the matrix (the write stream alone), half the modes and one wave of CTAs, and every class of sensors on its own --
@@ -162,7 +162,10 @@ def config_dict(wl, extra=None):
     return d
 
 
-def other_configs(spec: str) -> dict:
+T_START = time.time()
+
+
+def other_configs(spec: str, budget_s: float) -> dict:
     """Short device-resident runs of the other configurations (cold-L2 protocol, 10 steps), one process each so that
     nothing they do can take the headline run down; what the line keeps of each: step time, columns/s, roofline
     fractions, the dominant kernel and the parity spot check."""
@@ -171,6 +174,9 @@ def other_configs(spec: str) -> dict:
         cfg = tag.rstrip("rgp")
         if cfg not in ("1", "2", "3", "4", "5"):
             out[tag] = {"error": "unknown tag"}
+            continue
+        if time.time() - T_START > budget_s:      # the default run must end within minutes whatever the box is like
+            out[tag] = {"skipped": f"time budget: {budget_s:.0f} s since the start of bench.py were spent (--extra-budget-s)"}
             continue
         cmd = [sys.executable, os.path.abspath(__file__), "--config", cfg, "--steps", "10", "--warmup", "3", "--no-e2e",
                "--no-cpu-baseline", "--parity-modes", "32", "--extra", "none"]
@@ -182,7 +188,7 @@ def other_configs(spec: str) -> dict:
         if tag.endswith("p"):
             env["SYNIM_ZONAL_PACKED"] = "1"
         try:
-            res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
+            res = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT, env=env)
             last = [ln for ln in res.stdout.strip().splitlines() if ln.startswith("{")]
             if res.returncode != 0 or not last:
                 out[tag] = {"error": (res.stderr or res.stdout)[-400:]}
@@ -289,11 +295,13 @@ def main():
     ap.add_argument("--dictionary", type=int, default=0, metavar="MODES_PER_LAYER",
                     help="also run the 12-layer dictionary of PAPER.md:132 (workloads.make_dictionary, this many modes per "
                          "layer) through synim_dictionary_host and report it under config.dictionary")
-    ap.add_argument("--extra", default="2,4,5,3r,3g,3p,4p",
+    ap.add_argument("--extra", default="5,4,2,3p,4p,3g,3r",
                     help="at N=1, after the timed run: short device-resident runs of these other configurations, each in its "
                          "own process, reported under config.other_configs ('3r' = config 3 with edge repair, '3g' = config 3 "
                          "with the G-tilt estimator, '3p' / '4p' = config 3 / 4 through the opt-in packed zonal walk, SYNIM_ZONAL_PACKED=1; "
                          "'none' to skip)")
+    ap.add_argument("--extra-budget-s", type=float, default=200.0,
+                    help="no further --extra child is started once bench.py has been running this long (reported as skipped)")
     ap.add_argument("--no-ablate", action="store_true",
                     help="skip config.ablation: after the timed run, a few cold steps each of (a) a plain fill of the matrix "
                          "(the write stream alone), (b) half the modes, and one wave of CTAs for zonal modes, (c) every class of "
@@ -598,7 +606,7 @@ def main():
         if e2e_error:
             line["e2e"] = {"value": None, "unit": UNIT, "error": e2e_error}
         if world == 1 and args.extra.strip().lower() != "none":
-            line["config"]["other_configs"] = other_configs(args.extra)
+            line["config"]["other_configs"] = other_configs(args.extra, args.extra_budget_s)
         if world == 1 and not args.no_cpu_baseline:
             v, cores, desc = oracle_throughput(wl, 10.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}

@@ -133,6 +133,8 @@ int64_t synim_row_offset(const synim_geometry *geom, int32_t wfs);
  *                synim_create_geometry); anything else is INVALID_ARG
  *   d_out        DEVICE float32, column-major, ld >= synim_num_rows(); every element of rows
  *                [0, num_rows) of columns [0, n_modes) is written (padding rows are left untouched)
+ *                n_modes == 0, or a geometry without any valid subaperture (num_rows == 0), is a no-op that
+ *                returns SYNIM_OK whatever the buffers are
  * Errors: INVALID_ARG (NULL, n_modes < 0, ld < rows, singular affine), ALIGNMENT, CUDA. */
 synim_status synim_interaction_matrix(const synim_geometry *geom, const float *d_influence, int32_t n_modes,
                                       const int32_t *d_bbox, const int32_t *d_diag, int32_t bbox_max_w,

@@ -470,6 +470,7 @@ static synim_status run_interaction_matrix(const synim_geometry *g, const float 
         if (cur != g->device)
             return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: current device %d is not the geometry's device %d", cur, g->device);
     }
+    if (g->rows == 0) return SYNIM_OK;   // no sensor has a valid subaperture: the matrix has no rows, nothing is read or written
     if (!d_influence || !d_out) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: NULL device buffer");
     if (ld < g->rows) return fail(SYNIM_ERR_INVALID_ARG, "synim_interaction_matrix: ld = %lld < rows = %lld", (long long)ld, g->rows);
     if (reinterpret_cast<uintptr_t>(d_influence) % 16 != 0)

@@ -355,6 +355,13 @@ def test_empty_and_degenerate_inputs(S):
                                             S._affine_array(S.affines_of(wl), None), 0, small.data_ptr(),
                                             geom.num_rows - 1, None) == S.ERR_INVALID_ARG
     geom.destroy()
+    # sensors without any valid subaperture: a matrix without rows, a no-op whatever the output pointer is
+    blind = W.WfsInput(2, 4, np.ones((8, 8), np.float32), np.zeros((2, 2), np.uint8), W.physical())
+    geom = S.create_geometry(wl.ny, wl.nx, [blind])
+    assert geom.num_rows == 0
+    out = S.interaction_matrix(geom, cube, None, [S.compose_affine(blind.phys)])
+    assert out.shape == (wl.n_modes, 0)
+    geom.destroy()
     # a valid subaperture without light is refused at geometry creation
     dark = W.WfsInput(2, 4, np.zeros((8, 8), np.float32), np.ones((2, 2), np.uint8), W.physical())
     with pytest.raises(S.SynimError) as e:

@@ -81,6 +81,15 @@ def test_strip_kernel_zonal_modes(emu):
     s = [W.WfsInput(10, 6, pup, W.valid_subaps(pup, 10, 6), W.physical(rot_deg=10.0, mag_x=0.4, mag_y=0.4))]
     wl = W.Workload("split supports", 0, 160, 160, cube, W.tight_bboxes(cube), s)
     check(emu.interaction_matrix(wl, hint=False), O.interaction_matrix(wl), wl)
+    # a geometry without any valid subaperture: a matrix without rows, a no-op whatever the output pointer is
+    import ctypes
+    import harness
+    blind = W.WfsInput(10, 6, pup, np.zeros((10, 10), np.uint8), W.physical())
+    h, keep = emu.geometry([blind], 160, 160)
+    assert emu.L.synim_num_rows(h) == 0
+    arr = harness.S._affine_array(emu.affines([blind]), [1.0])
+    assert emu.L.synim_interaction_matrix(h, emu.reg(cube).ctypes.data, 2, None, None, 0, 0, arr, 0, None, 0, None) == 0
+    emu.L.synim_destroy(h)
 
 
 def test_flat_one_shot_entry_point(emu):

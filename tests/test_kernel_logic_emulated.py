@@ -340,3 +340,24 @@ def test_seeded_random_cases_against_the_oracle(emu):
     if n >= 64:      # the campaign reaches every path: compact / dense x estimator x repair
         assert {(False, 0, None), (True, 0, None), (False, 1, None), (True, 1, None)} <= kinds
         assert any(k[2] == "binary" for k in kinds) and any(k[2] == "soft" for k in kinds)
+
+
+@pytest.mark.skipif(not os.environ.get("SYNIM_EMU_FULL"), reason="opt-in (about 25 minutes): SYNIM_EMU_FULL=1")
+@pytest.mark.timeout(7200)
+def test_full_size_configurations_whole_matrices(emu):
+    """The bodies of the full-size GPU tests (tests/test_gpu_parity.py::_full_size) through the emulated library: the WHOLE
+    matrices of configs 2, 3 and 4 and the 256 seeded modes of config 5 the GPU test draws, by the GPU tests' own rule
+    (assert_parity).  Round 2, last commit: 6.0e-7, 4.9e-6, 6.9e-6 and 1.05e-6 of the column maximum."""
+    import test_gpu_parity as T
+    for cfg, n_sample, chunk in ((2, None, 256), (3, None, 256), (4, None, 256), (5, 256, 16)):
+        wl = W.make_config(cfg)
+        sel = np.arange(wl.n_modes)
+        if n_sample is not None:
+            sel = np.sort(np.random.default_rng(15).choice(wl.n_modes, size=n_sample, replace=False))
+        worst = 0.0
+        for c0 in range(0, len(sel), chunk):
+            idx = sel[c0:c0 + chunk]
+            sub = W.Workload(wl.name, wl.cfg, wl.ny, wl.nx, np.ascontiguousarray(wl.cube[idx]),
+                             None if wl.bbox is None else np.ascontiguousarray(wl.bbox[idx]), wl.wfs)
+            worst = max(worst, T.assert_parity(emu.interaction_matrix(sub).astype(np.float32), O.interaction_matrix(sub), sub)[1])
+        print(f"config {cfg}: {len(sel)} modes x {len(wl.wfs)} sensors, worst elementwise error {worst:.2e}")

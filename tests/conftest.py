@@ -19,7 +19,7 @@ def pytest_configure(config):
 # The order inside a class is the files' own; tests that need no GPU are not touched.
 _GPU_FIRST = ("test_config1_", "test_config2_", "test_config3_", "test_config4_", "test_compute_bboxes", "test_octagon_")
 _GPU_LATER = (
-    ("test_host_", "test_dictionary_host", "test_mode_ranges_through", "test_flat_one_shot"),
+    ("test_host_", "test_dictionary_host", "test_mode_ranges_through", "test_flat_one_shot", "test_one_geometry_many"),
     ("test_edge_repair", "test_packed_zonal", "test_projection_matrix"),
     ("test_seeded_random_cases",),
     ("test_debug_build",),

@@ -550,6 +550,33 @@ def test_dictionary_host_streams_layers_with_their_own_grids(S, monkeypatch):
     geom.destroy()
 
 
+def test_one_geometry_many_transforms(S):
+    """The on-line regime (what bench.py times): the geometry is built once and the transforms change from
+    call to call -- compact and dense modes, both estimators, a map that comes back (the tile plans are memoised per
+    sensor and map).  Every call against the oracle."""
+    import dataclasses
+    import torch
+    base = W.make_config(1, max_modes=10)
+    geom = S.create_geometry(base.ny, base.nx, base.wfs)
+    cube = torch.from_numpy(base.cube).cuda()
+    bbox, diag = S.compute_supports(cube)
+    bmax = S.bbox_extent(bbox)
+    out = torch.empty((base.n_modes, geom.num_rows), dtype=torch.float32, device="cuda")
+    maps = [dict(), dict(rot_deg=31.0, mag_x=0.9, mag_y=1.1), dict(shift_x=2.5, shift_y=-1.25), dict(rot_deg=31.0, mag_x=0.9, mag_y=1.1),
+            dict(rot_deg=-120.0, mag_x=1.2, mag_y=1.2, shift_x=-0.4)]
+    for dense in (False, True):
+        for k, phys in enumerate(maps):
+            mode = k % 2 if k else 0
+            wfs = [dataclasses.replace(w, phys=W.physical(**phys), slope_scale=1.0 + 0.5 * k) for w in base.wfs]
+            wl = W.Workload(f"call {k}", 0, base.ny, base.nx, base.cube, None if dense else base.bbox, wfs)
+            out.fill_(float("nan"))
+            S.interaction_matrix(geom, cube, None if dense else bbox, S.affines_of(wl), [w.slope_scale for w in wfs], out=out,
+                                 bbox_max=(0, 0) if dense else bmax, diag=None if dense else diag, mode=mode)
+            torch.cuda.synchronize()
+            assert_parity(out.cpu().numpy().T, O.interaction_matrix(wl, mode=O.GTILT if mode else O.ND), wl)
+    geom.destroy()
+
+
 def test_flat_one_shot_entry_point(S):
     """synim_interaction_matrix_flat (north_star's argument list: create -> supports -> matrix -> destroy in one call)
     gives the matrix of the piecewise calls bit for bit, and meets the bar on its own."""

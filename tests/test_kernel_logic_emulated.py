@@ -361,3 +361,38 @@ def test_full_size_configurations_whole_matrices(emu):
                              None if wl.bbox is None else np.ascontiguousarray(wl.bbox[idx]), wl.wfs)
             worst = max(worst, T.assert_parity(emu.interaction_matrix(sub).astype(np.float32), O.interaction_matrix(sub), sub)[1])
         print(f"config {cfg}: {len(sel)} modes x {len(wl.wfs)} sensors, worst elementwise error {worst:.2e}")
+
+
+def test_one_geometry_many_transforms(emu):
+    """The on-line regime (what bench.py times): the geometry is built once and the transforms change from
+    call to call -- compact and dense modes, both estimators, a map that comes back (the tile plans are memoised per
+    sensor and map).  Every call against the oracle."""
+    import ctypes
+    import dataclasses
+    import harness
+    L = emu.L
+    base = W.make_config(1, max_modes=10)
+    h, keep = emu.geometry(base.wfs, base.ny, base.nx)
+    rows = int(L.synim_num_rows(h))
+    cube = emu.reg(np.ascontiguousarray(base.cube))
+    bbox = emu.reg(np.zeros((base.n_modes, 4), np.int32))
+    diag = emu.reg(np.zeros((base.n_modes, 4), np.int32))
+    emu.chk(L.synim_compute_bboxes(cube.ctypes.data, base.n_modes, base.ny, base.nx, bbox.ctypes.data, diag.ctypes.data, None))
+    bw, bh = ctypes.c_int32(), ctypes.c_int32()
+    emu.chk(L.synim_bbox_extent(bbox.ctypes.data, base.n_modes, ctypes.byref(bw), ctypes.byref(bh), None))
+    out = emu.reg(np.empty((base.n_modes, rows), np.float32))
+    maps = [dict(), dict(rot_deg=31.0, mag_x=0.9, mag_y=1.1), dict(shift_x=2.5, shift_y=-1.25), dict(rot_deg=31.0, mag_x=0.9, mag_y=1.1),
+            dict(rot_deg=-120.0, mag_x=1.2, mag_y=1.2, shift_x=-0.4)]
+    for dense in (False, True):
+        for k, phys in enumerate(maps):
+            mode = k % 2 if k else 0                       # both estimators along the way
+            wfs = [dataclasses.replace(w, phys=W.physical(**phys), slope_scale=1.0 + 0.5 * k) for w in base.wfs]
+            wl = W.Workload(f"call {k}", 0, base.ny, base.nx, base.cube, None if dense else base.bbox, wfs)
+            arr = harness.S._affine_array(emu.affines(wfs), [w.slope_scale for w in wfs])
+            out[:] = np.nan
+            emu.chk(L.synim_interaction_matrix(h, cube.ctypes.data, base.n_modes, None if dense else bbox.ctypes.data,
+                                               None if dense else diag.ctypes.data, 0 if dense else bw.value, 0 if dense else bh.value,
+                                               arr, mode, out.ctypes.data, rows, None))
+            assert np.isfinite(out).all()
+            check(out.T.astype(np.float64), O.interaction_matrix(wl, mode=O.GTILT if mode else O.ND), wl)
+    L.synim_destroy(h)

@@ -78,3 +78,32 @@ def test_product_code_never_touches_the_oracle():
                 assert "liboracle" not in text and "import oracle" not in text and "from oracle" not in text, f
     otext = open(os.path.join(ROOT, "oracle", "oracle.py")).read() + open(os.path.join(ROOT, "oracle", "synim_oracle.c")).read()
     assert "libsynim" not in otext and "paper_2606_07759_b200" not in otext.replace("paper_2606_07759_b200/csrc", "")
+
+
+def test_header_is_plain_c_and_links_from_c(tmp_path):
+    """include/synim.h is the boundary: it compiles as strict C11 and as C++17, and a C program that includes it links
+    against the library and reaches the entry points that need no GPU (version, argument errors, NULL-safe destroy)."""
+    import shutil
+    import subprocess
+    hdr = os.path.join(ROOT, "include", "synim.h")
+    subprocess.check_call(["gcc", "-std=c11", "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only", "-x", "c", hdr])
+    subprocess.check_call(["g++", "-std=c++17", "-Wall", "-Werror", "-fsyntax-only", "-x", "c++", hdr])
+    src = tmp_path / "use.c"
+    src.write_text(
+        '#include "synim.h"\n#include <stdio.h>\n#include <string.h>\n'
+        "int main(void) {\n"
+        "  synim_wfs_affine a; synim_wfs_physical p; memset(&p, 0, sizeof p);\n"
+        "  if (synim_version() != SYNIM_VERSION_MAJOR * 1000 + SYNIM_VERSION_MINOR) return 1;\n"
+        "  if (synim_compose_affine(&p, &a) != SYNIM_ERR_INVALID_ARG) return 2;   /* zero magnification */\n"
+        "  if (strlen(synim_last_error()) == 0) return 3;\n"
+        "  if (synim_num_rows(NULL) != -1) return 4;\n"
+        "  synim_destroy(NULL);\n"
+        "  if (synim_interaction_matrix(NULL, NULL, 0, NULL, NULL, 0, 0, NULL, SYNIM_SLOPES_ND, NULL, 0, NULL) != SYNIM_ERR_INVALID_ARG) return 5;\n"
+        '  printf("ok %d\\n", (int)synim_version());\n  return 0;\n}\n')
+    exe = tmp_path / "use"
+    shutil.copy(synim.LIB_PATH, tmp_path / "libsynim.so")
+    subprocess.check_call(["gcc", "-std=c11", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe),
+                           "-L", str(tmp_path), "-lsynim", "-Wl,-rpath," + str(tmp_path)])
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0, (out.returncode, out.stdout, out.stderr)
+    assert out.stdout.startswith("ok ")

@@ -20,8 +20,8 @@ workload: BASELINE.json config C (default 3: ELT MCAO ground DM, 5065 actuators 
   cpu_baseline  the float64 oracle, as it stands, on the host cores, on a bounded sample of modes
 
 --repair times synim_interaction_matrix_repaired (edge repair) on the config's modes cut by a
-source-frame mask; --dictionary M adds the 12-layer dictionary of PAPER.md:132 (M modes per layer) through
-synim_dictionary_host under config.dictionary.
+source-frame mask; --dictionary M (default 64; 0 to skip) adds, at N=1, the 12-layer dictionary of PAPER.md:132 (M modes per
+layer) through synim_dictionary_host under config.dictionary.
 --extra (default "5,4,2,3p,4p,3g,3r", most wanted first): at N=1 the line also carries, under config.other_configs, short device-resident runs
 of the other configurations, each in its own process.
 config.ablation (and other_configs[*].ablation; --no-ablate to skip): after everything else, a few cold steps each of a plain
@@ -292,9 +292,9 @@ def main():
     ap.add_argument("--repair", action="store_true",
                     help="time synim_interaction_matrix_repaired (edge repair, PAPER.md:69-76) on the config's modes cut by "
                          "a source-frame pupil mask instead of the plain hot path")
-    ap.add_argument("--dictionary", type=int, default=0, metavar="MODES_PER_LAYER",
-                    help="also run the 12-layer dictionary of PAPER.md:132 (workloads.make_dictionary, this many modes per "
-                         "layer) through synim_dictionary_host and report it under config.dictionary")
+    ap.add_argument("--dictionary", type=int, default=64, metavar="MODES_PER_LAYER",
+                    help="at N=1 also run the 12-layer dictionary of PAPER.md:132 (workloads.make_dictionary, this many modes per "
+                         "layer) through synim_dictionary_host and report it under config.dictionary (0: skip)")
     ap.add_argument("--extra", default="5,4,2,3p,4p,3g,3r",
                     help="at N=1, after the timed run: short device-resident runs of these other configurations, each in its "
                          "own process, reported under config.other_configs ('3r' = config 3 with edge repair, '3g' = config 3 "
@@ -508,9 +508,19 @@ def main():
         if e2e_error is None:
             e2e = (e2e_ms, h2d, d2h, host_in, e2e_parity)
 
-    # the multi-layer dictionary of PAPER.md:132-138, end to end through host buffers (optional)
+    # what the step time is made of (N = 1; a side leg: reported, never fatal)
+    ablation = None
+    if world == 1 and not args.no_ablate and not args.repair:
+        try:
+            ablation = ablate(synim, wl, geom, cube, bbox, diag, bmax, affines, scales, out, scratch, stream, smode,
+                              float(cold.mean()))
+        except Exception as exc:
+            ablation = {"error": f"{type(exc).__name__}: {exc}"}
+
+    # the multi-layer dictionary of PAPER.md:132-138, end to end through host buffers (the very last device work: a
+    # side leg that fails here can hurt nothing else)
     dictionary = None
-    if args.dictionary > 0 and rank == 0:
+    if args.dictionary > 0 and world == 1 and not os.environ.get("SYNIM_BENCH_CHILD"):
         try:
             layers = workloads.make_dictionary(n_layers=12, max_modes=args.dictionary)
             dgeom = synim.create_geometry(layers[0].ny, layers[0].nx, layers[0].wfs)
@@ -539,15 +549,6 @@ def main():
             dgeom.destroy()
         except Exception as exc:       # (a side leg: reported, never fatal)
             dictionary = {"error": f"{type(exc).__name__}: {exc}"}
-
-    # what the step time is made of (N = 1; the last device work of the run; a side leg: reported, never fatal)
-    ablation = None
-    if world == 1 and not args.no_ablate and not args.repair:
-        try:
-            ablation = ablate(synim, wl, geom, cube, bbox, diag, bmax, affines, scales, out, scratch, stream, smode,
-                              float(cold.mean()))
-        except Exception as exc:
-            ablation = {"error": f"{type(exc).__name__}: {exc}"}
 
     # max over ranks (one process: no device work here, so that a side leg that failed above cannot take the line down)
     times = [float(cold.mean()), e2e[0] if e2e else 0.0, float(warm.mean()), strong_ms]

@@ -316,11 +316,14 @@ def interaction_matrix_flat(cube, wfs: Sequence, affines: Sequence[Sequence[floa
     assert cube.is_cuda and cube.dtype == torch.float32 and cube.is_contiguous() and cube.dim() == 3
     n, ny, nx = (int(v) for v in cube.shape)
     grids = (WfsGrid * len(wfs))()
-    keep, rows = [], 0
+    keep, rows, on_device = [], 0, {}
     for k, w in enumerate(wfs):
         valid = np.ascontiguousarray(w.valid, dtype=np.uint8)
-        pupil = w.pupil if isinstance(w.pupil, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(w.pupil, dtype=np.float32))
-        pupil = pupil.to(device="cuda", dtype=torch.float32).contiguous()
+        pupil = on_device.get(id(w.pupil))     # the SAME pupil object -> the same device buffer -> shared maps (as in Geometry)
+        if pupil is None:
+            pupil = w.pupil if isinstance(w.pupil, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(w.pupil, dtype=np.float32))
+            pupil = pupil.to(device="cuda", dtype=torch.float32).contiguous()
+            on_device[id(w.pupil)] = pupil
         keep.append((valid, pupil))
         grids[k].n_subap, grids[k].n_pix = int(w.n_subap), int(w.n_pix)
         grids[k].valid_mask = valid.ctypes.data

@@ -114,10 +114,13 @@ class Emu:
         L = self.L
         n = len(wl.wfs)
         grids = (S.WfsGrid * n)()
-        keep = []
+        keep, shared = [], {}
         for k, w in enumerate(wl.wfs):
             valid = np.ascontiguousarray(w.valid, dtype=np.uint8)
-            pupil = self.reg(np.ascontiguousarray(w.pupil, dtype=np.float32).copy())
+            pupil = shared.get(id(w.pupil))      # (sensors that pass the same buffer share their maps, as in geometry())
+            if pupil is None:
+                pupil = self.reg(np.ascontiguousarray(w.pupil, dtype=np.float32).copy())
+                shared[id(w.pupil)] = pupil
             keep.append((valid, pupil))
             grids[k].n_subap, grids[k].n_pix = int(w.n_subap), int(w.n_pix)
             grids[k].valid_mask = valid.ctypes.data

@@ -95,11 +95,11 @@ def test_strip_kernel_zonal_modes(emu):
 def test_flat_one_shot_entry_point(emu):
     """synim_interaction_matrix_flat (north_star's argument list: create -> supports -> matrix -> destroy) gives the
     matrix of the piecewise calls bit for bit, compact and dense, both estimators."""
-    wl = W.make_config(1, max_modes=16)
+    wl = W.make_config(1, max_modes=5)
     assert np.array_equal(emu.interaction_matrix_flat(wl), emu.interaction_matrix(wl))
     assert np.array_equal(emu.interaction_matrix_flat(wl, compact=False), emu.interaction_matrix(wl, use_bbox=False))
     check(emu.interaction_matrix_flat(wl, mode=1), O.interaction_matrix(wl, mode=O.GTILT), wl)
-    wl = W.make_config(4, max_modes=4)
+    wl = W.make_config(4, max_modes=2)        # sensors of two classes: two launches inside the one call
     check(emu.interaction_matrix_flat(wl), O.interaction_matrix(wl), wl)
 
 
